@@ -1,0 +1,122 @@
+/*
+ * mpdiv.h -- C ABI of libmpdiv.so: batched exact division of midsize unsigned integers on one
+ * NVIDIA B200 (sm_100a), after "On GPU Implementation for Multi-Precision Integer Division"
+ * (arxiv/paper_2606_06386; citations are lines of the paper text PAPER.md).
+ *
+ * Method: one division per thread block; quotient by Newton iteration on Watt's whole shifted
+ * inverse shinv_h(v) = floor(B^h / v) (Definition 1; Alg. 1-2),
+ * then the +-1 quotient / remainder correction of Alg. 3 (Theorem 2 :156-162).
+ * B = 2^32.  All arithmetic is exact integer arithmetic.
+ *
+ * Conventions common to every entry point
+ *   - Numbers are little-endian arrays of uint32 limbs: limb j has weight B^j.
+ *     Batches are row-major: instance i of an operand with stride s starts at ptr + i*s.
+ *     A value shorter than its stride is zero padded at the top; the kernels find the effective
+ *     precision themselves ("Prec").
+ *   - Pointers of the *_batch functions are DEVICE pointers owned by the caller (PyTorch allocates
+ *     them); they must be 16-byte aligned and every stride must be a multiple of 4 limbs.
+ *     Outputs must not overlap inputs.  The library allocates no persistent memory, never frees
+ *     caller memory and never synchronises the stream: work is enqueued on `stream` and the call
+ *     returns.  The first call of each kernel sets its shared-memory attribute (host side only).
+ *   - Return value: MPDIV_OK, or an error code; nothing is enqueued when an error is returned.
+ *     No exception crosses the ABI.  mpdiv_strerror() gives a text for a code.
+ *   - Supported sizes: strides up to MPDIV_MAX_LIMBS limbs (2^18 bits, the paper's range,
+ *     PAPER.md:194); any effective precision inside the stride, including 0.
+ */
+#ifndef MPDIV_H
+#define MPDIV_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* binary-compatible with cudaStream_t (0 / NULL = the legacy default stream) */
+typedef struct CUstream_st *mpdiv_stream_t;
+
+#define MPDIV_MAX_LIMBS 8192
+
+enum {
+    MPDIV_OK = 0,
+    MPDIV_ERR_BAD_ARG = 1,      /* null pointer, non-positive size, misaligned pointer or stride */
+    MPDIV_ERR_UNSUPPORTED = 2,  /* stride above MPDIV_MAX_LIMBS, or shared memory budget exceeded */
+    MPDIV_ERR_CUDA = 3          /* a CUDA runtime call failed (launch, attribute, copy) */
+};
+
+/*
+ * Division, Alg. 3: for each i < batch
+ *     q_i = floor(u_i / v_i),   r_i = u_i - q_i * v_i        (u = q*v + r, 0 <= r < v)
+ *   u : batch x u_limbs (device, read)      v : batch x v_limbs (device, read), v_limbs <= u_limbs
+ *   q : batch x u_limbs (device, written)   r : batch x v_limbs (device, written)
+ * q has stride u_limbs because the quotient of an M-limb by an n-limb number can need M-n+1
+ * limbs, and up to M when the divisor is short; both outputs are zero padded.
+ * v_i = 0 (undefined in the paper) does not trap: q_i is set to all ones, r_i to the
+ * low v_limbs limbs of u_i, and the instance is counted in mpdiv_debug_counters.
+ */
+int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
+                uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
+
+/*
+ * Multiplication, the unit of the paper's cost model (PAPER.md:105-106 MULT / MULTMOD, :166, :186):
+ *     c_i = (a_i * b_i) mod B^c_limbs
+ *   a : batch x a_limbs, b : batch x b_limbs (device, read);  c : batch x c_limbs (device, written)
+ * c_limbs = a_limbs + b_limbs gives the full product; a smaller c_limbs gives the truncated
+ * ("close") product, whose skipped limb products are not computed.  c_limbs <= a_limbs + b_limbs.
+ */
+int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs,
+                uint32_t *c, int c_limbs, int batch, mpdiv_stream_t stream);
+
+/*
+ * Whole shifted inverse as the division uses it, Alg. 1-2 and Theorem 2
+ * (PAPER.md:160):   w_i = floor(B^h / v_i) + lambda_i,  lambda_i in {0, 1}
+ * i.e. the UNCORRECTED Newton result, so that its time is the "2..4 multiplications" of the cost
+ * model.   v : batch x v_limbs (device, read);  w : batch x w_limbs (device, written),
+ * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_LIMBS.  v_i = 0 gives w_i = all ones (counted as an error).
+ */
+int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
+                int batch, mpdiv_stream_t stream);
+
+/*
+ * Host-buffer form of mpdiv_batch for end-to-end use: u, v, q, r are HOST pointers (pinned memory
+ * recommended); `workspace` is a caller-owned DEVICE buffer of at least
+ * mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch) bytes.  Enqueues H2D copies of u and v, the
+ * division, and D2H copies of q and r on `stream`, then returns; the caller synchronises.
+ */
+size_t mpdiv_host_workspace_bytes(int u_limbs, int v_limbs, int batch);
+int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host, int v_limbs,
+                     uint32_t *q_host, uint32_t *r_host, int batch,
+                     void *workspace, size_t workspace_bytes, mpdiv_stream_t stream);
+
+/*
+ * Integer-multiply roofline probe: every thread of a full-occupancy grid runs
+ * `iters` rounds of independent 32x32+64 multiply-accumulate chains (kind 0: IMAD.WIDE with carry
+ * chain, the instruction the multiplier uses; kind 1: plain mad.lo 32-bit), no memory traffic.
+ * Writes one checksum word per thread to `sink` (device, >= mpdiv_imad_probe_threads() words) and
+ * stores the number of limb products issued per launch in *products (host).  Time it with events.
+ */
+int mpdiv_imad_probe_threads(void);
+int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *products,
+                     mpdiv_stream_t stream);
+
+/*
+ * Debug counters accumulated by every mpdiv_batch / shinv_batch launch since the last reset
+ * (device-side atomics on a library-owned 64-byte buffer; reading them synchronises `stream`):
+ *   out[0] instances with the delta = -1 correction (u < v*q0)
+ *   out[1] instances with one delta = +1 correction
+ *   out[2] instances needing more than one +1 step (outside Theorem 2's range; expected 0)
+ *   out[3] one-limb divisors      out[4] u < v early exits      out[5] v = 0 instances
+ *   out[6] Newton steps that took the negative branch of PowDiff (sign = 0)
+ *   out[7] divisors that are an exact power of B (Alg. 1 line 9)
+ */
+int mpdiv_debug_counters(unsigned long long out[8], int reset, mpdiv_stream_t stream);
+
+/* "mpdiv <version> sm_100a ..." */
+const char *mpdiv_version(void);
+const char *mpdiv_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPDIV_H */

@@ -1,0 +1,180 @@
+"""Python binding of libmpdiv.so (include/mpdiv.h): argument marshalling only.
+
+Every function takes torch CUDA tensors (dtype int32 or uint32, contiguous, batch x limbs,
+little-endian limbs) that the CALLER allocates, passes their ``data_ptr()`` and the current
+CUDA stream to the C ABI, and returns the output tensors.  No arithmetic happens here and
+there is no CPU fallback: if the library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+_LIB = None
+_VOIDP = ctypes.c_void_p
+
+OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
+MAX_LIMBS = 8192
+
+
+class MpdivError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__("%s: status %d (%s)" % (what, code, strerror(code)))
+        self.code = code
+
+
+def lib() -> ctypes.CDLL:
+    """Load libmpdiv.so (must have been built: ``python -m paper_2606_06386_b200.build``)."""
+    global _LIB
+    if _LIB is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(
+                "libmpdiv.so is not built (%s); run __graft_entry__.build() -- there is no CPU fallback" % path)
+        L = ctypes.CDLL(path)
+        i, sz = ctypes.c_int, ctypes.c_size_t
+        L.mpdiv_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
+        L.mpmul_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, _VOIDP]
+        L.shinv_batch.argtypes = [_VOIDP, i, i, _VOIDP, i, i, _VOIDP]
+        L.mpdiv_host_workspace_bytes.argtypes = [i, i, i]
+        L.mpdiv_host_workspace_bytes.restype = sz
+        L.mpdiv_batch_host.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP, sz, _VOIDP]
+        L.mpdiv_imad_probe_threads.argtypes = []
+        L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
+        L.mpdiv_debug_counters.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), i, _VOIDP]
+        L.mpdiv_version.restype = ctypes.c_char_p
+        L.mpdiv_strerror.argtypes = [i]
+        L.mpdiv_strerror.restype = ctypes.c_char_p
+        for name in ("mpdiv_batch", "mpmul_batch", "shinv_batch", "mpdiv_batch_host",
+                     "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_debug_counters"):
+            getattr(L, name).restype = i
+        _LIB = L
+    return _LIB
+
+
+EXPORTS = ("mpdiv_batch", "mpmul_batch", "shinv_batch", "mpdiv_host_workspace_bytes",
+           "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
+           "mpdiv_debug_counters", "mpdiv_version", "mpdiv_strerror")
+
+
+def version() -> str:
+    return lib().mpdiv_version().decode()
+
+
+def strerror(code: int) -> str:
+    return lib().mpdiv_strerror(int(code)).decode()
+
+
+def _stream_ptr(stream=None) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _check_dev(t: torch.Tensor, name: str):
+    if not t.is_cuda:
+        raise ValueError("%s must be a CUDA tensor" % name)
+    if t.dtype not in (torch.int32, torch.uint32):
+        raise ValueError("%s must be int32/uint32" % name)
+    if t.dim() != 2 or not t.is_contiguous():
+        raise ValueError("%s must be a contiguous (batch, limbs) tensor" % name)
+
+
+def _raise(code: int, what: str):
+    if code != OK:
+        raise MpdivError(code, what)
+
+
+def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
+                r: torch.Tensor | None = None, stream=None):
+    """q = floor(u / v), r = u - q*v per row.  q has u's shape, r has v's shape."""
+    _check_dev(u, "u")
+    _check_dev(v, "v")
+    batch, ul = u.shape
+    vl = v.shape[1]
+    if v.shape[0] != batch:
+        raise ValueError("batch mismatch")
+    if q is None:
+        q = torch.empty_like(u)
+    if r is None:
+        r = torch.empty_like(v)
+    _check_dev(q, "q")
+    _check_dev(r, "r")
+    if tuple(q.shape) != (batch, ul) or tuple(r.shape) != (batch, vl):
+        raise ValueError("q must be (batch, u_limbs) and r (batch, v_limbs)")
+    _raise(lib().mpdiv_batch(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
+                             _stream_ptr(stream)), "mpdiv_batch")
+    return q, r
+
+
+def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor | None = None, stream=None):
+    """c = (a * b) mod B^c_limbs per row."""
+    _check_dev(a, "a")
+    _check_dev(b, "b")
+    batch = a.shape[0]
+    if b.shape[0] != batch:
+        raise ValueError("batch mismatch")
+    if c is None:
+        c = torch.empty((batch, c_limbs), dtype=a.dtype, device=a.device)
+    _check_dev(c, "c")
+    _raise(lib().mpmul_batch(a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], c.data_ptr(), c_limbs, batch,
+                             _stream_ptr(stream)), "mpmul_batch")
+    return c
+
+
+def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = None, stream=None):
+    """w = floor(B^h / v) + lambda, lambda in {0, 1}, per row (the uncorrected Newton result)."""
+    _check_dev(v, "v")
+    batch = v.shape[0]
+    if w is None:
+        w = torch.empty((batch, w_limbs), dtype=v.dtype, device=v.device)
+    _check_dev(w, "w")
+    _raise(lib().shinv_batch(v.data_ptr(), v.shape[1], int(h), w.data_ptr(), w_limbs, batch,
+                             _stream_ptr(stream)), "shinv_batch")
+    return w
+
+
+def host_workspace_bytes(u_limbs: int, v_limbs: int, batch: int) -> int:
+    return int(lib().mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch))
+
+
+def mpdiv_batch_host(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor, r: torch.Tensor,
+                     workspace: torch.Tensor, stream=None):
+    """Host-buffer form: u, v, q, r are (pinned) CPU tensors, workspace a CUDA byte tensor.
+    Enqueues H2D + division + D2H on the stream; the caller synchronises."""
+    for t, name in ((u, "u"), (v, "v"), (q, "q"), (r, "r")):
+        if t.is_cuda or not t.is_contiguous() or t.dtype not in (torch.int32, torch.uint32):
+            raise ValueError("%s must be a contiguous int32/uint32 CPU tensor" % name)
+    if not workspace.is_cuda:
+        raise ValueError("workspace must be a CUDA tensor")
+    batch, ul = u.shape
+    vl = v.shape[1]
+    _raise(lib().mpdiv_batch_host(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
+                                  workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                  _stream_ptr(stream)), "mpdiv_batch_host")
+    return q, r
+
+
+def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=None):
+    """Launch the integer-multiply probe; returns (limb products issued, sink tensor)."""
+    n = lib().mpdiv_imad_probe_threads()
+    if n <= 0:
+        raise MpdivError(ERR_CUDA, "mpdiv_imad_probe_threads")
+    if sink is None:
+        sink = torch.empty(n, dtype=torch.int32, device="cuda")
+    prod = ctypes.c_ulonglong(0)
+    _raise(lib().mpdiv_imad_probe(sink.data_ptr(), int(kind), int(iters), ctypes.byref(prod),
+                                  _stream_ptr(stream)), "mpdiv_imad_probe")
+    return int(prod.value), sink
+
+
+COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b")
+
+
+def debug_counters(reset: bool = False, stream=None) -> dict:
+    out = (ctypes.c_ulonglong * 8)()
+    _raise(lib().mpdiv_debug_counters(out, 1 if reset else 0, _stream_ptr(stream)), "mpdiv_debug_counters")
+    return {k: int(out[i]) for i, k in enumerate(COUNTER_NAMES)}

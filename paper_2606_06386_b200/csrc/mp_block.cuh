@@ -1,0 +1,277 @@
+// Block-level multi-precision primitives for sm_100a (one big integer per thread block).
+//
+// Numbers are little-endian arrays of 32-bit limbs held in shared memory for the whole
+// division ("the remaining computation uses fast memory").  Every buffer is zero
+// padded to a multiple of TILE limbs so that the multiplier can always read whole tiles.
+//
+// Linear-cost operations (PAPER.md 3.2-3.3): each thread owns 8 consecutive limbs, resolves
+// carries sequentially inside them with add.cc/addc.cc chains and publishes a 2-bit
+// (generate, propagate) code -- the CarryOP code of PAPER.md:343-358, :440.  Unlike the
+// paper's shuffle scan (Listing 1.6) the codes of a warp are gathered with
+// two ballots and the prefix is computed by ONE integer addition: adding the words G|P and G
+// ripples a carry through exactly the propagate bits, so (sum ^ (G|P) ^ G) holds the carry
+// into every lane.  The same trick over the per-warp codes finishes the block, with a single
+// __syncthreads per operation.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace mpd {
+
+typedef uint32_t limb;
+constexpr int TILE = 8;        // limbs per multiplier tile edge
+constexpr int CHUNK = 8;       // limbs per thread in linear operations
+
+__host__ __device__ constexpr int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// Per-block bookkeeping for the scans/reductions: a double-buffered word per warp.
+struct BlkScratch {
+    uint32_t code[2][32];
+};
+
+struct Blk {
+    BlkScratch *sc;
+    uint32_t parity;   // which half of sc->code the next collective uses
+};
+
+// ---------------------------------------------------------------------------------------
+// block collectives
+// ---------------------------------------------------------------------------------------
+template <int T>
+__device__ __forceinline__ int block_max(int v, Blk &blk)
+{
+    constexpr int NW = T / 32;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = __reduce_max_sync(0xffffffffu, v);
+    volatile uint32_t *code = blk.sc->code[blk.parity & 1];
+    blk.parity++;
+    if (lane == 0) code[warp] = (uint32_t)v;
+    __syncthreads();
+    int r = (lane < NW) ? (int)code[lane] : INT32_MIN;
+    return __reduce_max_sync(0xffffffffu, r);
+}
+
+// Carry/borrow prefix over the block.  Thread t contributes g (its chunk generates a carry) and
+// p (its chunk propagates an incoming carry), never both; cin enters below thread 0.
+// Returns the carry into this thread's chunk; cout = carry out of the last thread.
+template <int T>
+__device__ __forceinline__ uint32_t carry_scan(uint32_t g, uint32_t p, uint32_t cin, Blk &blk,
+                                               uint32_t &cout)
+{
+    constexpr int NW = T / 32;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t G = __ballot_sync(0xffffffffu, g != 0);
+    const uint32_t P = __ballot_sync(0xffffffffu, p != 0);
+    const uint32_t a = G | P, b = G;
+    const uint32_t wg = (uint32_t)(((uint64_t)a + b) >> 32);   // warp generates
+    const uint32_t wp = (P == 0xffffffffu) ? 2u : 0u;          // warp propagates
+    volatile uint32_t *code = blk.sc->code[blk.parity & 1];
+    blk.parity++;
+    if (lane == 0) code[warp] = wg | wp;
+    __syncthreads();
+    const uint32_t c = (lane < NW) ? code[lane] : 0u;
+    const uint64_t GW = __ballot_sync(0xffffffffu, (c & 1u) != 0);
+    const uint64_t PW = __ballot_sync(0xffffffffu, (c & 2u) != 0);
+    const uint64_t aw = GW | PW, bw = GW;
+    const uint64_t cw = (aw + bw + cin) ^ aw ^ bw;             // bit w = carry into warp w
+    cout = (uint32_t)(cw >> NW) & 1u;
+    const uint32_t cwarp = (uint32_t)(cw >> warp) & 1u;
+    const uint32_t cl = (a + b + cwarp) ^ a ^ b;               // bit l = carry into lane l
+    return (cl >> lane) & 1u;
+}
+
+// ---------------------------------------------------------------------------------------
+// 8-limb chunk arithmetic (in registers)
+// ---------------------------------------------------------------------------------------
+// r = a + b, returns carry out
+__device__ __forceinline__ uint32_t add8(limb (&r)[8], const limb (&a)[8], const limb (&b)[8])
+{
+    uint32_t c;
+    asm("add.cc.u32 %0, %9, %17;\n\t"
+        "addc.cc.u32 %1, %10, %18;\n\t"
+        "addc.cc.u32 %2, %11, %19;\n\t"
+        "addc.cc.u32 %3, %12, %20;\n\t"
+        "addc.cc.u32 %4, %13, %21;\n\t"
+        "addc.cc.u32 %5, %14, %22;\n\t"
+        "addc.cc.u32 %6, %15, %23;\n\t"
+        "addc.cc.u32 %7, %16, %24;\n\t"
+        "addc.u32 %8, 0, 0;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
+          "=r"(r[7]), "=r"(c)
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]), "r"(a[7]),
+          "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]), "r"(b[4]), "r"(b[5]), "r"(b[6]), "r"(b[7]));
+    return c;
+}
+
+// r = a - b, returns borrow out (0/1)
+__device__ __forceinline__ uint32_t sub8(limb (&r)[8], const limb (&a)[8], const limb (&b)[8])
+{
+    uint32_t c;
+    asm("sub.cc.u32 %0, %9, %17;\n\t"
+        "subc.cc.u32 %1, %10, %18;\n\t"
+        "subc.cc.u32 %2, %11, %19;\n\t"
+        "subc.cc.u32 %3, %12, %20;\n\t"
+        "subc.cc.u32 %4, %13, %21;\n\t"
+        "subc.cc.u32 %5, %14, %22;\n\t"
+        "subc.cc.u32 %6, %15, %23;\n\t"
+        "subc.cc.u32 %7, %16, %24;\n\t"
+        "subc.u32 %8, 0, 0;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
+          "=r"(r[7]), "=r"(c)
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]), "r"(a[7]),
+          "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]), "r"(b[4]), "r"(b[5]), "r"(b[6]), "r"(b[7]));
+    return c & 1u;
+}
+
+// r += c (c small), returns carry out
+__device__ __forceinline__ uint32_t inc8(limb (&r)[8], uint32_t cin)
+{
+    uint32_t c;
+    asm("add.cc.u32 %0, %0, %9;\n\t"
+        "addc.cc.u32 %1, %1, 0;\n\t"
+        "addc.cc.u32 %2, %2, 0;\n\t"
+        "addc.cc.u32 %3, %3, 0;\n\t"
+        "addc.cc.u32 %4, %4, 0;\n\t"
+        "addc.cc.u32 %5, %5, 0;\n\t"
+        "addc.cc.u32 %6, %6, 0;\n\t"
+        "addc.cc.u32 %7, %7, 0;\n\t"
+        "addc.u32 %8, 0, 0;"
+        : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]),
+          "+r"(r[7]), "=r"(c)
+        : "r"(cin));
+    return c;
+}
+
+// r -= c (c in {0,1}), returns borrow out
+__device__ __forceinline__ uint32_t dec8(limb (&r)[8], uint32_t cin)
+{
+    uint32_t c;
+    asm("sub.cc.u32 %0, %0, %9;\n\t"
+        "subc.cc.u32 %1, %1, 0;\n\t"
+        "subc.cc.u32 %2, %2, 0;\n\t"
+        "subc.cc.u32 %3, %3, 0;\n\t"
+        "subc.cc.u32 %4, %4, 0;\n\t"
+        "subc.cc.u32 %5, %5, 0;\n\t"
+        "subc.cc.u32 %6, %6, 0;\n\t"
+        "subc.cc.u32 %7, %7, 0;\n\t"
+        "subc.u32 %8, 0, 0;"
+        : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]),
+          "+r"(r[7]), "=r"(c)
+        : "r"(cin));
+    return c & 1u;
+}
+
+__device__ __forceinline__ bool all_eq8(const limb (&r)[8], limb x)
+{
+    return ((r[0] ^ x) | (r[1] ^ x) | (r[2] ^ x) | (r[3] ^ x) | (r[4] ^ x) | (r[5] ^ x) |
+            (r[6] ^ x) | (r[7] ^ x)) == 0;
+}
+
+// ---------------------------------------------------------------------------------------
+// linear operations on shared-memory numbers
+// ---------------------------------------------------------------------------------------
+// dst[i] = fa(i) +/- fb(i) +/- carry for i in [0, len), len a multiple of 8.  fa/fb return the
+// limb of each operand at index i (0 outside the operand): shifts by whole limbs
+// (shift_n) are folded into these index maps instead of being
+// materialised.  Map-scan-map of PAPER.md:423-432.  Returns the final carry (borrow).
+// dst may alias an operand only when that operand is read at the same index it is written.
+// Ends with a __syncthreads: dst is visible to the whole block on return.
+template <int T, bool SUB, class FA, class FB>
+__device__ __forceinline__ uint32_t lin_addsub(limb *dst, int len, FA fa, FB fb, uint32_t cin,
+                                               Blk &blk)
+{
+    for (int base = 0; base < len; base += CHUNK * T) {
+        const int i0 = base + CHUNK * (int)threadIdx.x;
+        limb a[8], b[8], r[8];
+        const bool active = i0 < len;
+        uint32_t g = 0, p = active ? 0u : 1u;   // idle threads pass the carry on to the block's cout
+        if (active) {
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                a[j] = fa(i0 + j);
+                b[j] = fb(i0 + j);
+            }
+            if (SUB) {
+                g = sub8(r, a, b);
+                p = all_eq8(r, 0u);
+            } else {
+                g = add8(r, a, b);
+                p = all_eq8(r, 0xffffffffu);
+            }
+        }
+        uint32_t cout;
+        const uint32_t c = carry_scan<T>(g, p, cin, blk, cout);
+        if (active) {
+            if (SUB) dec8(r, c); else inc8(r, c);
+            uint4 *d4 = reinterpret_cast<uint4 *>(dst + i0);
+            d4[0] = make_uint4(r[0], r[1], r[2], r[3]);
+            d4[1] = make_uint4(r[4], r[5], r[6], r[7]);
+        }
+        cin = cout;
+    }
+    __syncthreads();
+    return cin;
+}
+
+// limb i of a number stored at p with n valid limbs, read at index i + off (0 outside)
+struct LimbView {
+    const limb *p;
+    int n;
+    int off;
+    __device__ __forceinline__ limb operator()(int i) const
+    {
+        const int j = i + off;
+        return (j >= 0 && j < n) ? p[j] : 0u;
+    }
+};
+struct NotView {   // ~x over [0, n), 0 outside: used for B^n - x = ~x + 1.
+    const limb *p; // x has `valid` readable limbs (zero beyond)
+    int n;
+    int valid;
+    __device__ __forceinline__ limb operator()(int i) const
+    {
+        return (i < n) ? ~((i < valid) ? p[i] : 0u) : 0u;
+    }
+};
+struct ZeroView {
+    __device__ __forceinline__ limb operator()(int) const { return 0u; }
+};
+
+// dst[0..len) = src[i + off] (0 outside [0, n)); len multiple of 4.  Whole-limb shift / masked copy.
+template <int T>
+__device__ __forceinline__ void lin_copy(limb *dst, int len, const limb *src, int n, int off)
+{
+    for (int i = threadIdx.x; i < len; i += T) {
+        const int j = i + off;
+        dst[i] = (j >= 0 && j < n) ? src[j] : 0u;
+    }
+    __syncthreads();
+}
+
+template <int T>
+__device__ __forceinline__ void lin_zero(limb *dst, int len)
+{
+    for (int i = threadIdx.x; i < len; i += T) dst[i] = 0u;
+    __syncthreads();
+}
+
+// any limb of a[lo, hi) non-zero?  (block-uniform result)
+template <int T>
+__device__ __forceinline__ bool any_nonzero(const limb *a, int lo, int hi)
+{
+    uint32_t acc = 0;
+    for (int i = lo + (int)threadIdx.x; i < hi; i += T) acc |= a[i];
+    return __syncthreads_or(acc != 0) != 0;
+}
+
+// number of significant limbs of a[0, n)  ("prec")
+template <int T>
+__device__ __forceinline__ int prec_of(const limb *a, int n, Blk &blk)
+{
+    int top = 0;
+    for (int i = threadIdx.x; i < n; i += T)
+        if (a[i] != 0u) top = i + 1;   // i increases, so the last hit is this thread's highest
+    return block_max<T>(top, blk);
+}
+
+}  // namespace mpd

@@ -1,0 +1,164 @@
+// Whole shifted inverse (Alg. 1-2) and division (Alg. 3) for
+// one big integer per thread block, operands resident in shared memory.
+//
+// Reading of the garbled Algorithm 1:
+//   * the loop runs  ceil(log2(H-1)) + 2  times with H = max(h-k, 2)            (printed bound)
+//   * guard digits g = 2; the final shift is -(g + H - (h-k))                   (PAPER.md:92 l.26-27)
+//   * Step's negative branch subtracts one more when the discarded low limbs of w*x are
+//     non-zero (floor of a negative number, eq. (2))
+//   * the divisor prefix drops s limbs with s rounded DOWN to a multiple of 4 so that the prefix
+//     stays 16-byte aligned in shared memory; a longer prefix is always admissible.
+//   * one-limb divisors (Alg. 1 l.6 "divide by 1 digit") are mapped to two-limb ones:
+//     floor(B^h / v) = floor(B^(h+1) / (v*B)), and (u*B) div (v*B) = u div v with remainder r*B.
+#pragma once
+#include "mp_mul.cuh"
+
+namespace mpd {
+
+// debug counters (include/mpdiv.h: mpdiv_debug_counters)
+__device__ unsigned long long g_counters[8];
+enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
+       CNT_SIGN_NEG, CNT_POW_B };
+
+__device__ __forceinline__ void count(int which)
+{
+    if (threadIdx.x == 0) atomicAdd(&g_counters[which], 1ull);
+}
+
+// significant limbs of a shared-memory number known to have at most `bound` limbs.
+// Every thread walks the same (stable) words, so the result is block-uniform.
+__device__ __forceinline__ int top_prec(const limb *a, int bound)
+{
+    while (bound > 0 && a[bound - 1] == 0u) --bound;
+    return bound;
+}
+
+struct UnitView {   // B^pos
+    int pos;
+    __device__ __forceinline__ limb operator()(int i) const { return i == pos ? 1u : 0u; }
+};
+
+// Shared-memory working set of one Shinv: two iterate buffers, x, and the product scratch.
+struct ShinvBufs {
+    limb *WA, *WB;   // iterates w (ping-pong); capacity >= round_up(H + 6, 8) limbs each
+    limb *X;         // |B^h'' - v'w|; capacity >= k + 48 limbs
+    limb *P;         // product; capacity >= h + 40 limbs
+    MulScratch ms;
+};
+
+// w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
+// The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
+template <int T>
+__device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk)
+{
+    limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
+    const MulScratch &ms = bufs.ms;
+    const int g = 2;
+
+    // ---- special cases (Alg. 1 lines 5-10) -------------------------------------
+    const bool low_nz = any_nonzero<T>(V, 0, k);
+    const limb vtop = V[k];
+    const bool pow_b = (vtop == 1u) && !low_nz;               // v = B^k
+    int special = -1;                                          // value of a one-limb result
+    if (k > h || (k == h && !pow_b)) special = 0;              // v > B^h
+    else if (!pow_b && k == h - 1 &&
+             (vtop > 0x80000000u || (vtop == 0x80000000u && low_nz))) special = 1;   // 2v > B^h
+    if (special >= 0) {
+        for (int i = threadIdx.x; i < TILE; i += T) WA[i] = (i == 0) ? (limb)special : 0u;
+        __syncthreads();
+        return 1;
+    }
+    if (pow_b) {                                               // v = B^k  ->  B^(h-k)
+        count(CNT_POW_B);
+        const int len = round_up(h - k + 1, TILE);
+        for (int i = threadIdx.x; i < len; i += T) WA[i] = (i == h - k) ? 1u : 0u;
+        __syncthreads();
+        return h - k + 1;
+    }
+
+    // ---- initial approximation (Alg. 1 lines 11-13): w = B^3 quo (v[k-1] + v[k] B), l = 2 ----
+    const int H = max(h - k, 2);
+    const int iters = ((H - 1 > 1) ? (32 - __clz(H - 2)) : 0) + 2;
+    limb *Wc = ((iters + 1) & 1) ? WB : WA;                    // so that write number iters+1 hits WA
+    limb *Wn = (Wc == WA) ? WB : WA;
+    if (threadIdx.x == 0) {
+        const unsigned long long V2 = ((unsigned long long)V[k] << 32) | V[k - 1];
+        const unsigned __int128 w0 = (((unsigned __int128)1) << 96) / V2;
+        Wc[0] = 0u; Wc[1] = 0u;                                // shift_g(w), g = 2 (Alg. 1 line 17)
+        Wc[2] = (limb)w0; Wc[3] = (limb)(w0 >> 32); Wc[4] = (limb)(w0 >> 64);
+        Wc[5] = 0u; Wc[6] = 0u; Wc[7] = 0u;
+    }
+    __syncthreads();
+    int l = 2;
+    int wlen = TILE;                                           // valid (zero padded) words of Wc
+
+    // ---- Refine (Alg. 1 lines 15-28) ------------------------------------------------------------
+    for (int it = 0; it < iters; ++it) {
+        const int m = min(H + 1 - l, l);
+        int s = max(0, k - 2 * l + 1 - g);
+        s &= ~3;                                               // keep the divisor prefix 16-byte aligned
+        const limb *Vp = V + s;                                // shift_{-s}(v)
+        const int pv = k + 1 - s;
+        const int hp = k + l + m - s + g;                      // h' of Step
+        const int hpp = hp - m;                                // h'' of PowDiff
+        const int pw = top_prec(Wc, min(wlen, l + g + 2));
+
+        // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
+        const int L = pv + pw - (l - g) + 1;
+        bool positive;
+        int xl;                                                // limbs of x (upper bound)
+        if (L >= hpp) {
+            // no room to truncate: full product and a comparison with B^h''
+            mul_full<T>(Vp, pv, Wc, pw, P, ms, blk);
+            const int pl = round_up(pv, TILE) + round_up(pw, TILE);
+            positive = !any_nonzero<T>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
+            if (positive) {
+                xl = hpp;                                      // x = B^h'' - p = ~p + 1 over h'' limbs
+                lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, pl}, ZeroView{}, 1u, blk);
+                // p = 0 cannot happen (v', w > 0); p = B^h'' exactly falls in the other branch
+            } else {
+                xl = pv + pw;                                  // x = p - B^h''
+                lin_addsub<T, true>(X, round_up(xl, TILE), LimbView{P, pl, 0}, UnitView{hpp}, 0u, blk);
+            }
+        } else {
+            // close product: only the L low limbs of v'w (MULTMOD)
+            mul_low<T>(Vp, pv, Wc, pw, L, P, ms, blk);
+            positive = P[L - 1] != 0u;                         // top limb set: v'w just below B^h''
+            xl = L;
+            if (positive)
+                lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, xl}, ZeroView{}, 1u, blk);
+            else
+                lin_copy<T>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
+        }
+        if (!positive) count(CNT_SIGN_NEG);
+        xl = top_prec(X, xl);
+
+        // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
+        const int d = hp - 2 * m;                              // limbs of w*x that the shift drops
+        const int nlen = round_up(l + m + g + 2, TILE);
+        if (xl == 0) {
+            lin_copy<T>(Wn, nlen, Wc, wlen, 1 - m);
+        } else {
+            mul_full<T>(Wc, pw, X, xl, P, ms, blk);
+            const int tl = round_up(pw, TILE) + round_up(xl, TILE);
+            if (positive) {
+                lin_addsub<T, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, 1 + d}, 0u, blk);
+            } else {
+                // floor of a negative: borrow one when any dropped limb (0..d) of w*x is non-zero
+                const uint32_t bin = any_nonzero<T>(P, 0, min(d + 1, tl)) ? 1u : 0u;
+                lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, 1 + d}, bin, blk);
+            }
+        }
+        l = l + m - 1;
+        wlen = nlen;
+        limb *t = Wc; Wc = Wn; Wn = t;
+    }
+
+    // ---- final shift_{-g - (H - (h-k))} (Alg. 1 lines 26-27) -------------------------------------
+    const int sh = g + (H - (h - k));
+    const int rlen = round_up(h - k + 2, TILE);
+    lin_copy<T>(Wn, rlen, Wc, wlen, sh);                       // Wn == WA by construction
+    return h - k + 1;
+}
+
+}  // namespace mpd

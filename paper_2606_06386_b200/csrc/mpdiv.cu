@@ -1,0 +1,258 @@
+// libmpdiv.so -- kernels and C ABI (include/mpdiv.h).  sm_100a only.
+#include <cstdint>
+#include <cstdio>
+#include <cuda_runtime.h>
+
+#include "../../include/mpdiv.h"
+#include "mp_block.cuh"
+#include "mp_mul.cuh"
+#include "mp_div.cuh"
+
+using namespace mpd;
+
+#define MPDIV_VERSION_STR "mpdiv 0.1 sm_100a (B200) limbs=u32 tile=8x8 imad.wide"
+
+// ---------------------------------------------------------------------------------------
+// global <-> shared staging
+// ---------------------------------------------------------------------------------------
+// dst[0..n) = src[0..n) with 128-bit coalesced loads (n multiple of 4), dst[n..pad) = 0.
+template <int T>
+__device__ __forceinline__ void load_number(limb *dst, const limb *__restrict__ src, int n, int pad)
+{
+    const uint4 *s4 = reinterpret_cast<const uint4 *>(src);
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+    for (int i = threadIdx.x; i < n / 4; i += T) d4[i] = __ldg(s4 + i);
+    for (int i = n + (int)threadIdx.x; i < pad; i += T) dst[i] = 0u;
+}
+
+// dst[0..n) = (i < valid) ? src[i] : 0, 128-bit coalesced stores; valid multiple of 4 not required.
+template <int T>
+__device__ __forceinline__ void store_number(limb *__restrict__ dst, const limb *src, int n, int valid)
+{
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+    for (int i = threadIdx.x; i < n / 4; i += T) {
+        const int b = 4 * i;
+        uint4 x;
+        x.x = (b + 0 < valid) ? src[b + 0] : 0u;
+        x.y = (b + 1 < valid) ? src[b + 1] : 0u;
+        x.z = (b + 2 < valid) ? src[b + 2] : 0u;
+        x.w = (b + 3 < valid) ? src[b + 3] : 0u;
+        d4[i] = x;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// mpmul_batch
+// ---------------------------------------------------------------------------------------
+struct MulLayout {
+    int a_off, b_off, p_off, hi_off, ov_off, c3_off, sc_off, total_words;
+};
+
+static MulLayout mul_layout(int a_limbs, int b_limbs, int c_limbs)
+{
+    MulLayout L;
+    const int pa = round_up(a_limbs, TILE) + TILE;
+    const int pb = round_up(b_limbs, TILE) + TILE;
+    const int full = round_up(a_limbs, TILE) + round_up(b_limbs, TILE);
+    const int pc = round_up(c_limbs < full ? c_limbs : full, TILE) + 2 * TILE;
+    int o = 0;
+    L.a_off = o; o += pa;
+    L.b_off = o; o += pb;
+    L.p_off = o; o += pc;
+    L.hi_off = o; o += pc;
+    L.ov_off = o; o += round_up(pc / TILE, 4);
+    L.c3_off = o; o += round_up(pc / TILE, 4);
+    L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
+    L.total_words = o;
+    return L;
+}
+
+template <int T>
+__global__ void __launch_bounds__(T)
+mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b, int b_limbs,
+             limb *__restrict__ c, int c_limbs, int batch, MulLayout L)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    limb *A = smem + L.a_off, *Bs = smem + L.b_off, *P = smem + L.p_off;
+    MulScratch ms{smem + L.hi_off, smem + L.ov_off, smem + L.c3_off};
+    Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
+
+    for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
+        load_number<T>(A, a + (size_t)inst * a_limbs, a_limbs, round_up(a_limbs, TILE) + TILE);
+        load_number<T>(Bs, b + (size_t)inst * b_limbs, b_limbs, round_up(b_limbs, TILE) + TILE);
+        __syncthreads();
+        const int na = prec_of<T>(A, a_limbs, blk);
+        const int nb = prec_of<T>(Bs, b_limbs, blk);
+        int valid = 0;
+        if (na > 0 && nb > 0) {
+            if (c_limbs >= na + nb) {
+                mul_full<T>(A, na, Bs, nb, P, ms, blk);
+                valid = round_up(na, TILE) + round_up(nb, TILE);
+            } else {
+                mul_low<T>(A, na, Bs, nb, c_limbs, P, ms, blk);
+                valid = c_limbs;
+            }
+        }
+        store_number<T>(c + (size_t)inst * c_limbs, P, c_limbs, valid);
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// integer-multiply roofline probe
+// ---------------------------------------------------------------------------------------
+constexpr int PROBE_THREADS = 256;
+constexpr int PROBE_BLOCKS_PER_SM = 4;
+
+template <int KIND>
+__global__ void __launch_bounds__(PROBE_THREADS)
+imad_probe_kernel(uint32_t *sink, int iters)
+{
+    if (KIND == 0) {
+        // the multiplier's own inner tile: 64 carry-chained IMAD.WIDE.U32 + 16 carry counters
+        DiagAcc s;
+        s.clear();
+        uint32_t a[8], b[8];
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+            a[j] = threadIdx.x * 2654435761u + j * 40503u + 1u;
+            b[j] = blockIdx.x * 2246822519u + j * 9973u + 7u;
+        }
+        for (int it = 0; it < iters; ++it) {
+            tile_mac(s, a, b);
+            a[0] ^= s.CY[0];   // keep the operands loop-variant without extra multiplies
+        }
+        uint32_t d[17];
+        diag_finish(s, d);
+        uint32_t x = 0;
+#pragma unroll
+        for (int j = 0; j < 17; j++) x ^= d[j];
+        sink[blockIdx.x * PROBE_THREADS + threadIdx.x] = x;
+    } else {
+        // 64 independent plain 32-bit IMADs per round (no carry, no wide result)
+        uint32_t acc[16];
+#pragma unroll
+        for (int j = 0; j < 16; j++) acc[j] = threadIdx.x + j;
+        uint32_t m = blockIdx.x * 2246822519u + 12345u;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 4; r++)
+#pragma unroll
+                for (int j = 0; j < 16; j++) acc[j] = acc[j] * m + acc[(j + 1) & 15];
+        }
+        uint32_t x = 0;
+#pragma unroll
+        for (int j = 0; j < 16; j++) x ^= acc[j];
+        sink[blockIdx.x * PROBE_THREADS + threadIdx.x] = x;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------
+namespace {
+
+int g_sm_count = 0;
+int g_max_smem = 0;
+
+bool device_props()
+{
+    if (g_sm_count > 0) return true;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return false;
+    if (cudaDeviceGetAttribute(&g_max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return false;
+    return g_sm_count > 0;
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// threads per block for a number of `limbs` limbs: one thread per 16 limbs, 64..512
+int threads_for(int limbs)
+{
+    int t = 64;
+    while (t < 512 && t * 16 < limbs) t *= 2;
+    return t;
+}
+
+template <class K>
+int set_smem(K kernel, size_t bytes)
+{
+    if ((int)bytes > g_max_smem) return MPDIV_ERR_UNSUPPORTED;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return MPDIV_ERR_CUDA;
+    }
+    return MPDIV_OK;
+}
+
+template <int T>
+int launch_mul(const limb *a, int a_limbs, const limb *b, int b_limbs, limb *c, int c_limbs, int batch,
+               cudaStream_t st)
+{
+    const MulLayout L = mul_layout(a_limbs, b_limbs, c_limbs);
+    const size_t bytes = (size_t)L.total_words * 4;
+    int rc = set_smem(mpmul_kernel<T>, bytes);
+    if (rc != MPDIV_OK) return rc;
+    mpmul_kernel<T><<<batch, T, bytes, st>>>(a, a_limbs, b, b_limbs, c, c_limbs, batch, L);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, uint32_t *c, int c_limbs,
+                int batch, mpdiv_stream_t stream)
+{
+    if (!a || !b || !c || a_limbs <= 0 || b_limbs <= 0 || c_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
+    if ((a_limbs | b_limbs | c_limbs) & 3) return MPDIV_ERR_BAD_ARG;
+    if (!aligned16(a) || !aligned16(b) || !aligned16(c)) return MPDIV_ERR_BAD_ARG;
+    if (c_limbs > a_limbs + b_limbs) return MPDIV_ERR_BAD_ARG;
+    if (a_limbs > MPDIV_MAX_LIMBS || b_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int big = a_limbs > b_limbs ? a_limbs : b_limbs;
+    switch (threads_for(2 * big)) {
+        case 64: return launch_mul<64>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
+        case 128: return launch_mul<128>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
+        case 256: return launch_mul<256>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
+        default: return launch_mul<512>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
+    }
+}
+
+int mpdiv_imad_probe_threads(void)
+{
+    if (!device_props()) return 0;
+    return g_sm_count * PROBE_BLOCKS_PER_SM * PROBE_THREADS;
+}
+
+int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *products, mpdiv_stream_t stream)
+{
+    if (!sink || iters <= 0 || (kind != 0 && kind != 1)) return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int blocks = g_sm_count * PROBE_BLOCKS_PER_SM;
+    if (kind == 0) imad_probe_kernel<0><<<blocks, PROBE_THREADS, 0, st>>>(sink, iters);
+    else imad_probe_kernel<1><<<blocks, PROBE_THREADS, 0, st>>>(sink, iters);
+    if (products) *products = (unsigned long long)blocks * PROBE_THREADS * 64ull * (unsigned long long)iters;
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+const char *mpdiv_version(void) { return MPDIV_VERSION_STR; }
+
+const char *mpdiv_strerror(int code)
+{
+    switch (code) {
+        case MPDIV_OK: return "ok";
+        case MPDIV_ERR_BAD_ARG: return "bad argument (null pointer, non-positive size, misaligned pointer or stride)";
+        case MPDIV_ERR_UNSUPPORTED: return "unsupported size (stride above MPDIV_MAX_LIMBS or shared memory budget exceeded)";
+        case MPDIV_ERR_CUDA: return "CUDA runtime error";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"
+
+#include "mpdiv_api.inl"

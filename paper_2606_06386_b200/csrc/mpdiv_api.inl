@@ -1,0 +1,334 @@
+// mpdiv_batch / shinv_batch kernels and the rest of the C ABI (included by mpdiv.cu).
+
+// ---------------------------------------------------------------------------------------
+// shared-memory arena of one division (word offsets).  Phases reuse the same words:
+//   Refine   : V | WB (=U area) | WA | X  P  HI  OV  C3            (u is not resident)
+//   quotient : V | U            | WA (= shinv, then q) | P  HI  OV  C3   (P up to 2M+2 limbs)
+// ---------------------------------------------------------------------------------------
+struct DivLayout {
+    int v_off, u_off, wa_off, big_off, sc_off, total_words;
+    int x_words;      // Refine: X at big_off, P behind it
+    int p_words_r;    // Refine: capacity of P and of HI
+    int p_words_q;    // quotient phase: capacity of P and of HI
+};
+
+// M: limbs of the dividend side (u stride, or h for shinv_batch); n: divisor stride;
+// with_quotient: reserve the 2M-limb product of u * shinv.
+static DivLayout div_layout(int M, int n, bool with_quotient)
+{
+    DivLayout L;
+    const int Mp = round_up(M, TILE);
+    const int np = round_up(n, TILE);
+    L.x_words = np + 48;
+    L.p_words_r = Mp + 48;
+    L.p_words_q = with_quotient ? 2 * Mp + 32 : 0;
+    const int ovr = round_up(L.p_words_r / TILE, 4), ovq = round_up(L.p_words_q / TILE, 4);
+    const int big_r = L.x_words + 2 * L.p_words_r + 2 * ovr;
+    const int big_q = 2 * L.p_words_q + 2 * ovq;
+    int o = 0;
+    L.v_off = o; o += np + 16;
+    L.u_off = o; o += Mp + 16;
+    L.wa_off = o; o += Mp + 16;
+    L.big_off = o; o += (big_r > big_q ? big_r : big_q);
+    L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
+    L.total_words = o;
+    return L;
+}
+
+__device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout &L)
+{
+    ShinvBufs b;
+    b.WA = smem + L.wa_off;
+    b.WB = smem + L.u_off;
+    b.X = smem + L.big_off;
+    b.P = b.X + L.x_words;
+    const int ov = round_up(L.p_words_r / TILE, 4);
+    b.ms.HI = b.P + L.p_words_r;
+    b.ms.OV = b.ms.HI + L.p_words_r;
+    b.ms.C3 = b.ms.OV + ov;
+    return b;
+}
+
+// ---------------------------------------------------------------------------------------
+// shinv_batch kernel
+// ---------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(T)
+shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
+             DivLayout L)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    limb *V = smem + L.v_off;
+    Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
+    const ShinvBufs bufs = refine_bufs(smem, L);
+    const int vpad = round_up(v_limbs, TILE) + 16;
+
+    for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
+        limb *wout = w + (size_t)inst * w_limbs;
+        load_number<T>(V + 4, v + (size_t)inst * v_limbs, v_limbs, vpad - 4);   // room to shift by one limb
+        if (threadIdx.x < 4) V[threadIdx.x] = 0u;
+        __syncthreads();
+        const int pv = prec_of<T>(V + 4, v_limbs, blk);
+        if (pv == 0) {                                   // v = 0: undefined
+            count(CNT_V_ZERO);
+            for (int i = threadIdx.x; i < w_limbs; i += T) wout[i] = 0xffffffffu;
+            __syncthreads();
+            continue;
+        }
+        int nw;
+        if (pv == 1) {                                   // one-limb divisor: Shinv(v*B, h+1)
+            count(CNT_ONE_LIMB);
+            if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }   // v*B at the (aligned) base V
+            __syncthreads();
+            nw = shinv_block<T>(V, 1, h + 1, bufs, blk);
+        } else {
+            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk);
+        }
+        store_number<T>(wout, bufs.WA, w_limbs, round_up(nw, TILE));
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// mpdiv_batch kernel: Alg. 3, one division per block
+// ---------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(T)
+mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
+             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
+    limb *U = smem + L.u_off;          // dividend at U + 4 (same)
+    limb *WA = smem + L.wa_off;        // shinv, then the quotient
+    Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
+    const ShinvBufs rb = refine_bufs(smem, L);
+    // quotient-phase product scratch
+    limb *PQ = smem + L.big_off;
+    MulScratch mq;
+    mq.HI = PQ + L.p_words_q;
+    mq.OV = mq.HI + L.p_words_q;
+    mq.C3 = mq.OV + round_up(L.p_words_q / TILE, 4);
+    const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
+
+    for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
+        const limb *ug = u + (size_t)inst * u_limbs;
+        limb *qg = q + (size_t)inst * u_limbs;
+        limb *rg = r + (size_t)inst * v_limbs;
+
+        // a1/a2: load, precisions ("h <- prec(u)")
+        load_number<T>(V + 4, v + (size_t)inst * v_limbs, v_limbs, vpad - 4);
+        load_number<T>(U + 4, ug, u_limbs, upad - 4);
+        if (threadIdx.x < 4) { V[threadIdx.x] = 0u; U[threadIdx.x] = 0u; }
+        __syncthreads();
+        const int pv = prec_of<T>(V + 4, v_limbs, blk);
+        int h = prec_of<T>(U + 4, u_limbs, blk);
+
+        if (pv == 0) {                                     // v = 0: q = all ones, r = low limbs of u
+            count(CNT_V_ZERO);
+            for (int i = threadIdx.x; i < u_limbs; i += T) qg[i] = 0xffffffffu;
+            store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
+            __syncthreads();
+            continue;
+        }
+        if (pv > h) {                                      // u < v: (0, u)
+            count(CNT_U_LT_V);
+            store_number<T>(qg, U + 4, u_limbs, 0);
+            store_number<T>(rg, U + 4, v_limbs, h);
+            __syncthreads();
+            continue;
+        }
+
+        // one-limb divisor: divide u*B by v*B (same quotient, remainder r*B)
+        const bool one_limb = (pv == 1);
+        const limb *Vb = V + 4;
+        limb *Ub = U + 4;
+        int k = pv - 1;
+        if (one_limb) {
+            count(CNT_ONE_LIMB);
+            if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }
+            __syncthreads();
+            Vb = V; k = 1; h = h + 1;
+        }
+
+        // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk);
+        const int psh = top_prec(WA, nw);
+
+        // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
+        if (one_limb) {
+            for (int i = threadIdx.x; i < upad; i += T)
+                U[i] = (i >= 1 && i <= u_limbs) ? __ldg(ug + i - 1) : 0u;
+            Ub = U;
+        } else {
+            load_number<T>(U + 4, ug, u_limbs, upad - 4);
+        }
+        __syncthreads();
+
+        // a9: q0 = shift_{-h}(u * shinv)  (Alg. 3 line 2); the full product, as printed
+        const int nq = h - k + 1;                          // q0 <= B^(h-k): at most h-k+1 limbs
+        const int qlen = round_up(nq + 1, TILE);
+        limb *Q = WA;
+        if (psh == 0) {
+            lin_zero<T>(Q, qlen);
+        } else {
+            mul_full<T>(Ub, h, WA, psh, PQ, mq, blk);
+            const int pl = round_up(h, TILE) + round_up(psh, TILE);
+            lin_copy<T>(Q, qlen, PQ, pl, h);               // WA (shinv) is dead: reuse it for q
+        }
+        const int pq = top_prec(Q, nq);
+
+        // a10: p = v * q0  (Alg. 3 line 3)
+        const int rlen = round_up(h + 1, TILE);            // p <= u + v < 2 B^h
+        int pl = 0;
+        if (pq > 0) {
+            mul_full<T>(Vb, k + 1, Q, pq, PQ, mq, blk);
+            pl = round_up(k + 1, TILE) + round_up(pq, TILE);
+        }
+
+        // a11: corrections (Alg. 3 lines 4-10, Theorem 2)
+        limb *R = PQ, *R2 = mq.HI;                         // r in place over p; HI is free after the product
+        uint32_t borrow = lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
+        if (borrow) {                                      // u < v*q0: delta = -1
+            count(CNT_DELTA_NEG);
+            lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
+            lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+        }
+        int plus = 0;
+        for (int step = 0; step < 4; ++step) {             // r >= v: delta = +1 (at most once by Theorem 2)
+            borrow = lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
+            if (borrow) break;
+            limb *t = R; R = R2; R2 = t;
+            lin_addsub<T, false>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+            ++plus;
+        }
+        if (plus == 1) count(CNT_DELTA_POS);
+        if (plus > 1) count(CNT_DELTA_MULTI);
+
+        // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
+        store_number<T>(qg, Q, u_limbs, min(qlen, u_limbs));
+        if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
+        else store_number<T>(rg, R, v_limbs, min(k + 1, v_limbs));
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// host side of mpdiv_batch / shinv_batch / host-buffer form / counters
+// ---------------------------------------------------------------------------------------
+namespace {
+
+template <int T>
+int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+               cudaStream_t st)
+{
+    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true);
+    const size_t bytes = (size_t)L.total_words * 4;
+    int rc = set_smem(mpdiv_kernel<T>, bytes);
+    if (rc != MPDIV_OK) return rc;
+    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+template <int T>
+int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st)
+{
+    const DivLayout L = div_layout(h + 1, v_limbs, false);
+    const size_t bytes = (size_t)L.total_words * 4;
+    int rc = set_smem(shinv_kernel<T>, bytes);
+    if (rc != MPDIV_OK) return rc;
+    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+int check_div_args(const void *u, int u_limbs, const void *v, int v_limbs, const void *q, const void *r,
+                   int batch)
+{
+    if (!u || !v || !q || !r || u_limbs <= 0 || v_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
+    if ((u_limbs | v_limbs) & 3) return MPDIV_ERR_BAD_ARG;
+    if (v_limbs > u_limbs) return MPDIV_ERR_BAD_ARG;
+    if (u_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    return MPDIV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
+                int batch, mpdiv_stream_t stream)
+{
+    int rc = check_div_args(u, u_limbs, v, v_limbs, q, r, batch);
+    if (rc != MPDIV_OK) return rc;
+    if (!aligned16(u) || !aligned16(v) || !aligned16(q) || !aligned16(r)) return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    switch (threads_for(u_limbs)) {
+        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st);
+        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st);
+        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st);
+        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st);
+    }
+}
+
+int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch,
+                mpdiv_stream_t stream)
+{
+    if (!v || !w || v_limbs <= 0 || w_limbs <= 0 || batch <= 0 || h < 1) return MPDIV_ERR_BAD_ARG;
+    if ((v_limbs | w_limbs) & 3) return MPDIV_ERR_BAD_ARG;
+    if (w_limbs < h + 1) return MPDIV_ERR_BAD_ARG;
+    if (!aligned16(v) || !aligned16(w)) return MPDIV_ERR_BAD_ARG;
+    if (h > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    switch (threads_for(h)) {
+        case 64: return launch_shinv<64>(v, v_limbs, h, w, w_limbs, batch, st);
+        case 128: return launch_shinv<128>(v, v_limbs, h, w, w_limbs, batch, st);
+        case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st);
+        default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st);
+    }
+}
+
+size_t mpdiv_host_workspace_bytes(int u_limbs, int v_limbs, int batch)
+{
+    if (u_limbs <= 0 || v_limbs <= 0 || batch <= 0) return 0;
+    return (size_t)batch * 2 * ((size_t)u_limbs + (size_t)v_limbs) * sizeof(uint32_t);
+}
+
+int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host, int v_limbs,
+                     uint32_t *q_host, uint32_t *r_host, int batch, void *workspace, size_t workspace_bytes,
+                     mpdiv_stream_t stream)
+{
+    int rc = check_div_args(u_host, u_limbs, v_host, v_limbs, q_host, r_host, batch);
+    if (rc != MPDIV_OK) return rc;
+    if (!workspace || !aligned16(workspace)) return MPDIV_ERR_BAD_ARG;
+    if (workspace_bytes < mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch)) return MPDIV_ERR_BAD_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const size_t ub = (size_t)batch * u_limbs * 4, vb = (size_t)batch * v_limbs * 4;
+    uint32_t *du = static_cast<uint32_t *>(workspace);
+    uint32_t *dv = du + (size_t)batch * u_limbs;
+    uint32_t *dq = dv + (size_t)batch * v_limbs;
+    uint32_t *dr = dq + (size_t)batch * u_limbs;
+    if (cudaMemcpyAsync(du, u_host, ub, cudaMemcpyHostToDevice, st) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyAsync(dv, v_host, vb, cudaMemcpyHostToDevice, st) != cudaSuccess) return MPDIV_ERR_CUDA;
+    rc = mpdiv_batch(du, u_limbs, dv, v_limbs, dq, dr, batch, stream);
+    if (rc != MPDIV_OK) return rc;
+    if (cudaMemcpyAsync(q_host, dq, ub, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyAsync(r_host, dr, vb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MPDIV_ERR_CUDA;
+    return MPDIV_OK;
+}
+
+int mpdiv_debug_counters(unsigned long long out[8], int reset, mpdiv_stream_t stream)
+{
+    if (!out) return MPDIV_ERR_BAD_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (cudaStreamSynchronize(st) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(out, g_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (reset) {
+        unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (cudaMemcpyToSymbol(g_counters, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    }
+    return MPDIV_OK;
+}
+
+}  // extern "C"
