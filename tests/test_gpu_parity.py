@@ -1,0 +1,207 @@
+"""Parity of the CUDA path (libmpdiv.so through the C ABI) with the CPU oracle -- bit exact.
+
+Every test here needs a B200 (``-m gpu``).  Inputs come from the seeded generators of
+``paper_2606_06386_b200.inputs``; expected values come from ``oracle/`` only.  q and r are
+unique, so every limb including the zero padding must match.  For shinv the
+two admissible values floor(B^h/v) + {0, 1} (Theorem 2) are both accepted.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2606_06386_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+NCPU = max(1, os.cpu_count() or 1)
+
+
+def dev(a: np.ndarray) -> torch.Tensor:
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.int32)).cuda()
+
+
+def host(t: torch.Tensor) -> np.ndarray:
+    return t.cpu().numpy().view(np.uint32)
+
+
+def gpu_div(u, v):
+    q, r = binding.mpdiv_batch(dev(u), dev(v))
+    torch.cuda.synchronize()
+    return host(q), host(r)
+
+
+def check_div(u, v, what=""):
+    q, r = gpu_div(u, v)
+    qo, ro = oracle.divmod_batch(u, v, threads=NCPU)
+    bad = np.nonzero((q != qo).any(axis=1) | (r != ro).any(axis=1))[0]
+    assert bad.size == 0, "%s: %d of %d instances differ, first %d" % (what, bad.size, u.shape[0], bad[0])
+
+
+# ------------------------------------------------------------------ multiplication
+@pytest.mark.parametrize("an,bn,cn", [
+    (4, 4, 8), (8, 8, 16), (12, 20, 32), (64, 64, 128), (512, 512, 1024), (516, 260, 776),
+    (1024, 1024, 2048), (2048, 1024, 3072), (4096, 4096, 8192), (8192, 4096, 12288),
+    (1024, 1024, 1024), (1024, 1024, 516), (2048, 2048, 1028), (4096, 4096, 4096), (520, 516, 524),
+    (64, 64, 4), (8192, 8192, 16384), (8192, 8192, 8192),
+])
+def test_mul_parity(an, bn, cn):
+    batch = 12
+    rng = inputs.rng_for(200, an % 65536)
+    a = inputs._uniform(rng, batch, an)
+    b = inputs._uniform(rng, batch, bn)
+    # ragged effective precisions, all-ones (worst carries) and zero operands
+    a[1, an // 2:] = 0
+    b[2, max(1, bn // 3):] = 0
+    a[3, :] = 0xFFFFFFFF
+    b[3, :] = 0xFFFFFFFF
+    a[4, :] = 0
+    b[5, :] = 0
+    a[6, 1:] = 0
+    b[7, 1:] = 0
+    a[8, :] = 0xFFFFFFFF
+    b[8, :] = 0
+    b[8, 0] = 1
+    c = host(binding.mpmul_batch(dev(a), dev(b), cn))
+    co = oracle.mul_batch(a, b, cn)
+    bad = np.nonzero((c != co).any(axis=1))[0]
+    assert bad.size == 0, "instances %s differ" % bad[:8]
+
+
+# ------------------------------------------------------------------ shifted inverse
+@pytest.mark.parametrize("vn,h", [(4, 7), (8, 16), (16, 17), (64, 128), (512, 1024), (1024, 2048),
+                                  (260, 777), (2048, 4096), (4096, 8192), (512, 512), (512, 300)])
+def test_shinv_parity(vn, h):
+    batch = 24
+    wn = (h + 1 + 3) // 4 * 4
+    _, v = inputs.directed(max(vn, 8), vn, count=batch, seed=inputs.SEED + h)
+    v2 = inputs._uniform(inputs.rng_for(201, h % 65536), 8, vn)
+    inputs._force_top_nonzero(v2)
+    v = np.concatenate([v, v2])
+    w = host(binding.shinv_batch(dev(v), h, wn))
+    wo = oracle.shinv_batch(v, h, wn)
+    lam_hist = {0: 0, 1: 0}
+    for i in range(v.shape[0]):
+        lam = inputs.from_limbs(w[i]) - inputs.from_limbs(wo[i])
+        assert lam in (0, 1), "instance %d: lambda = %d (Theorem 2 allows 0 or 1)" % (i, lam)
+        lam_hist[lam] += 1
+    print("lambda histogram", lam_hist)
+
+
+# ------------------------------------------------------------------ division: the five configs
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_div_config_full_size(cfg):
+    """BASELINE.json configs at full size, in the launch configuration bench.py times.
+
+    Configs 1-2 and 5 are checked on every instance; 3 and 4 (oracle: tens of ms per division)
+    on a seeded sample of instances, each compared limb by limb."""
+    u, v = inputs.config(cfg)
+    q, r = gpu_div(u, v)
+    batch = u.shape[0]
+    if cfg in (3, 4):
+        pick = np.sort(inputs.rng_for(300 + cfg).choice(batch, size=96 if cfg == 3 else 48, replace=False))
+    else:
+        pick = np.arange(batch)
+    qo, ro = oracle.divmod_batch(u[pick], v[pick], threads=NCPU)
+    bad = np.nonzero((q[pick] != qo).any(axis=1) | (r[pick] != ro).any(axis=1))[0]
+    assert bad.size == 0, "config %d: %d of %d checked instances differ (first: %d)" % (
+        cfg, bad.size, pick.size, pick[bad[0]])
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_div_config_invariants_all_instances(cfg):
+    """Properties that hold at any size, on EVERY instance of the big configs:
+    r < v limb-wise compare and u = q*v + r checked with Python integers (independent of both sides)."""
+    u, v = inputs.config(cfg)
+    q, r = gpu_div(u, v)
+    step = 1 if cfg == 3 else 1
+    for i in range(0, u.shape[0], step):
+        ui, vi = inputs.from_limbs(u[i]), inputs.from_limbs(v[i])
+        qi, ri = inputs.from_limbs(q[i]), inputs.from_limbs(r[i])
+        assert ri < vi and qi * vi + ri == ui, "instance %d" % i
+
+
+# ------------------------------------------------------------------ division: directed and ragged
+@pytest.mark.parametrize("M,n,count", [(8, 4, 256), (16, 8, 512), (32, 32, 512), (64, 32, 512),
+                                       (128, 64, 512), (1024, 512, 768), (2048, 1024, 384),
+                                       (2048, 2048, 384), (4096, 2048, 128), (8192, 4096, 48),
+                                       (8192, 8192, 32), (1028, 516, 256), (100, 52, 256)])
+def test_div_directed(M, n, count):
+    binding.debug_counters(reset=True)
+    u, v = inputs.directed(M, n, count=count)
+    check_div(u, v, "directed M=%d n=%d" % (M, n))
+    cnt = binding.debug_counters()
+    print("counters", cnt)
+    assert cnt["delta_multi"] == 0, "a quotient needed more than one +1 step (Theorem 2 violated)"
+
+
+def test_directed_reaches_corner_paths():
+    """The directed set must actually drive the rare branches: delta = -1, delta = +1,
+    the negative PowDiff sign, powers of B and one-limb divisors."""
+    binding.debug_counters(reset=True)
+    u, v = inputs.directed(64, 32, count=2048)
+    check_div(u, v, "directed 64/32")
+    cnt = binding.debug_counters(reset=True)
+    print("counters", cnt)
+    for key in ("delta_neg", "delta_pos", "sign_neg", "pow_b", "one_limb", "u_lt_v"):
+        assert cnt[key] > 0, "%s never fired" % key
+    assert cnt["delta_multi"] == 0
+
+
+@pytest.mark.parametrize("M", [64, 1024, 2048])
+def test_div_paper_shape(M):
+    """The paper's own workload shape: prec(u) = M-2, prec(v) uniform in 2..M/2."""
+    u, v = inputs.paper_shape(256, M)
+    check_div(u, v, "paper shape M=%d" % M)
+
+
+def test_div_random_effective_precisions():
+    """1000 randomised instances with random values and random effective precisions."""
+    rng = inputs.rng_for(400)
+    M = 256
+    us, vs = [], []
+    for _ in range(1000):
+        lu = int(rng.integers(0, M + 1))
+        lv = int(rng.integers(1, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, lv))
+    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions")
+
+
+def test_div_zero_divisor_does_not_trap():
+    binding.debug_counters(reset=True)
+    u, v = inputs.uniform_operands(8, 64, 32, config=77)
+    v[3] = 0
+    q, r = gpu_div(u, v)
+    assert (q[3] == 0xFFFFFFFF).all() and (r[3] == u[3, :32]).all()
+    keep = [0, 1, 2, 4, 5, 6, 7]
+    qo, ro = oracle.divmod_batch(u[keep], v[keep])
+    assert (q[keep] == qo).all() and (r[keep] == ro).all()
+    assert binding.debug_counters(reset=True)["v_zero"] == 1
+
+
+def test_host_buffer_form_matches():
+    u, v = inputs.config(1)
+    ut = torch.from_numpy(u.view(np.int32)).pin_memory()
+    vt = torch.from_numpy(v.view(np.int32)).pin_memory()
+    qt = torch.empty_like(ut).pin_memory()
+    rt = torch.empty_like(vt).pin_memory()
+    ws = torch.empty(binding.host_workspace_bytes(u.shape[1], v.shape[1], u.shape[0]), dtype=torch.uint8, device="cuda")
+    binding.mpdiv_batch_host(ut, vt, qt, rt, ws)
+    torch.cuda.synchronize()
+    qo, ro = oracle.divmod_batch(u, v, threads=NCPU)
+    assert (qt.numpy().view(np.uint32) == qo).all() and (rt.numpy().view(np.uint32) == ro).all()
+
+
+def test_bad_arguments_are_rejected():
+    u, v = inputs.uniform_operands(2, 8, 4, config=78)
+    du, dv = dev(u), dev(v)
+    with pytest.raises(binding.MpdivError) as e:
+        binding.mpdiv_batch(du[:, :6].contiguous(), dv)           # stride not a multiple of 4
+    assert e.value.code == binding.ERR_BAD_ARG
+    big = torch.zeros((1, 8196), dtype=torch.int32, device="cuda")
+    with pytest.raises(binding.MpdivError) as e:
+        binding.mpdiv_batch(big, dv[:1])
+    assert e.value.code == binding.ERR_UNSUPPORTED
