@@ -239,7 +239,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from paper_2606_06386_b200 import binding, inputs
+    from paper_2606_06386_b200 import binding, inputs, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -254,7 +254,7 @@ def run_ours(args):
     b, m, n = inputs.CONFIG_SHAPES[cfg]
     # weak scaling: every rank divides its own batch of the config's size (independent problems,
     # no data-path collective); rank r draws with seed SEED + r.
-    u, v = inputs.config(cfg, seed=inputs.SEED + rank)
+    u, v = inputs.config(cfg, seed=shard.rank_seed(inputs.SEED, rank))
     du, dv = to_dev(u), to_dev(v)
     q = torch.empty_like(du)
     r = torch.empty_like(dv)
@@ -275,13 +275,9 @@ def run_ours(args):
     barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
-    total_ms = float(sum(ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(float(sum(ms)), device="cuda")
     ms_per_step = total_ms / args.steps
-    value = world * b / (ms_per_step * 1e-3)
+    value = shard.aggregate_rate(b, world, ms_per_step)
 
     # ---- end to end: host buffers through mpdiv_batch_host (H2D + division + D2H inside the timing) ----
     hu = torch.from_numpy(u.view(np.int32)).pin_memory()
@@ -292,12 +288,8 @@ def run_ours(args):
     barrier()
     ms_e = time_steps(lambda: binding.mpdiv_batch_host(hu, hv, hq, hr, ws), args.steps, args.warmup, flush)
     barrier()
-    e_total = float(sum(ms_e))
-    if world > 1:
-        t = torch.tensor([e_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e_total = float(t.item())
-    e2e_value = world * b / (e_total / args.steps * 1e-3)
+    e_total = shard.max_over_ranks(float(sum(ms_e)), device="cuda")
+    e2e_value = shard.aggregate_rate(b, world, e_total / args.steps)
     io_bytes = b * 4 * (m + n)
     # the device-timed result and the host round trip must agree bit for bit (cheap self-consistency)
     same = bool((hq.cuda() == q).all().item() and (hr.cuda() == r).all().item())
