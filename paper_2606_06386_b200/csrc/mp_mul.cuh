@@ -27,38 +27,50 @@
 
 namespace mpd {
 
-// four limb products of one parity class of row a: (r0..r7) += a * (b0, b1, b2, b3) at limb
-// offsets 0, 2, 4, 6; the carry out of limb 7 is counted in cy.
-__device__ __forceinline__ void chain4(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3,
-                                       uint32_t &r4, uint32_t &r5, uint32_t &r6, uint32_t &r7,
+// four limb products of one parity class of row a: the 8-limb window held in the four 64-bit
+// accumulators (x0..x3) += a * (b0, b1, b2, b3) at limb offsets 0, 2, 4, 6; the carry out of the
+// window is counted in cy.  The accumulators are 64-bit registers so that ptxas keeps them in aligned
+// register pairs for the whole loop (with 32-bit halves it re-pairs them with moves and XOR swaps).
+__device__ __forceinline__ void chain4(uint64_t &x0, uint64_t &x1, uint64_t &x2, uint64_t &x3,
                                        uint32_t &cy, uint32_t a, uint32_t b0, uint32_t b1,
                                        uint32_t b2, uint32_t b3)
 {
-    asm("mad.lo.cc.u32 %0, %9, %10, %0;\n\t"
-        "madc.hi.cc.u32 %1, %9, %10, %1;\n\t"
-        "madc.lo.cc.u32 %2, %9, %11, %2;\n\t"
-        "madc.hi.cc.u32 %3, %9, %11, %3;\n\t"
-        "madc.lo.cc.u32 %4, %9, %12, %4;\n\t"
-        "madc.hi.cc.u32 %5, %9, %12, %5;\n\t"
-        "madc.lo.cc.u32 %6, %9, %13, %6;\n\t"
-        "madc.hi.cc.u32 %7, %9, %13, %7;\n\t"
-        "addc.u32 %8, %8, 0;"
-        : "+r"(r0), "+r"(r1), "+r"(r2), "+r"(r3), "+r"(r4), "+r"(r5), "+r"(r6), "+r"(r7), "+r"(cy)
+    asm("{\n\t"
+        ".reg .u32 l0, h0, l1, h1, l2, h2, l3, h3;\n\t"
+        "mov.b64 {l0, h0}, %0;\n\t"
+        "mov.b64 {l1, h1}, %1;\n\t"
+        "mov.b64 {l2, h2}, %2;\n\t"
+        "mov.b64 {l3, h3}, %3;\n\t"
+        "mad.lo.cc.u32 l0, %5, %6, l0;\n\t"
+        "madc.hi.cc.u32 h0, %5, %6, h0;\n\t"
+        "madc.lo.cc.u32 l1, %5, %7, l1;\n\t"
+        "madc.hi.cc.u32 h1, %5, %7, h1;\n\t"
+        "madc.lo.cc.u32 l2, %5, %8, l2;\n\t"
+        "madc.hi.cc.u32 h2, %5, %8, h2;\n\t"
+        "madc.lo.cc.u32 l3, %5, %9, l3;\n\t"
+        "madc.hi.cc.u32 h3, %5, %9, h3;\n\t"
+        "addc.u32 %4, %4, 0;\n\t"
+        "mov.b64 %0, {l0, h0};\n\t"
+        "mov.b64 %1, {l1, h1};\n\t"
+        "mov.b64 %2, {l2, h2};\n\t"
+        "mov.b64 %3, {l3, h3};\n\t"
+        "}"
+        : "+l"(x0), "+l"(x1), "+l"(x2), "+l"(x3), "+r"(cy)
         : "r"(a), "r"(b0), "r"(b1), "r"(b2), "r"(b3));
 }
 
-// Accumulators of one tile diagonal: E holds limbs 0..15, O limbs 1..14 (index = limb - 1),
-// CY the chain-end carries of limbs 8..16.
+// Accumulators of one tile diagonal: E[p] holds limbs 2p, 2p+1 (limbs 0..15), O[p] limbs 2p+1, 2p+2
+// (limbs 1..14), CY the chain-end carries of limbs 8..16.
 struct DiagAcc {
-    uint32_t E[16];
-    uint32_t O[14];
+    uint64_t E[8];
+    uint64_t O[7];
     uint32_t CY[9];
     __device__ __forceinline__ void clear()
     {
 #pragma unroll
-        for (int i = 0; i < 16; i++) E[i] = 0;
+        for (int i = 0; i < 8; i++) E[i] = 0;
 #pragma unroll
-        for (int i = 0; i < 14; i++) O[i] = 0;
+        for (int i = 0; i < 7; i++) O[i] = 0;
 #pragma unroll
         for (int i = 0; i < 9; i++) CY[i] = 0;
     }
@@ -68,19 +80,17 @@ template <int I>
 __device__ __forceinline__ void tile_row(DiagAcc &s, uint32_t a, const uint32_t (&b)[8])
 {
     if ((I & 1) == 0) {
-        // j even -> column i+j even -> E[i..i+7], carry into limb i+8
-        chain4(s.E[I], s.E[I + 1], s.E[I + 2], s.E[I + 3], s.E[I + 4], s.E[I + 5], s.E[I + 6],
-               s.E[I + 7], s.CY[I], a, b[0], b[2], b[4], b[6]);
-        // j odd -> column odd -> limbs i+1..i+8 = O[i..i+7], carry into limb i+9
-        chain4(s.O[I], s.O[I + 1], s.O[I + 2], s.O[I + 3], s.O[I + 4], s.O[I + 5], s.O[I + 6],
-               s.O[I + 7], s.CY[I + 1], a, b[1], b[3], b[5], b[7]);
+        constexpr int p = I / 2;
+        // j even -> limb i+j even -> E pairs p..p+3 (limbs i..i+7), carry into limb i+8
+        chain4(s.E[p], s.E[p + 1], s.E[p + 2], s.E[p + 3], s.CY[I], a, b[0], b[2], b[4], b[6]);
+        // j odd -> limbs i+1..i+8 = O pairs p..p+3, carry into limb i+9
+        chain4(s.O[p], s.O[p + 1], s.O[p + 2], s.O[p + 3], s.CY[I + 1], a, b[1], b[3], b[5], b[7]);
     } else {
-        // j even -> column odd -> limbs i..i+7 = O[i-1..i+6], carry into limb i+8
-        chain4(s.O[I - 1], s.O[I], s.O[I + 1], s.O[I + 2], s.O[I + 3], s.O[I + 4], s.O[I + 5],
-               s.O[I + 6], s.CY[I], a, b[0], b[2], b[4], b[6]);
-        // j odd -> column even -> limbs i+1..i+8 = E[i+1..i+8], carry into limb i+9
-        chain4(s.E[I + 1], s.E[I + 2], s.E[I + 3], s.E[I + 4], s.E[I + 5], s.E[I + 6], s.E[I + 7],
-               s.E[I + 8], s.CY[I + 1], a, b[1], b[3], b[5], b[7]);
+        constexpr int p = (I - 1) / 2;
+        // j even -> limbs i..i+7 = O pairs p..p+3, carry into limb i+8
+        chain4(s.O[p], s.O[p + 1], s.O[p + 2], s.O[p + 3], s.CY[I], a, b[0], b[2], b[4], b[6]);
+        // j odd -> limbs i+1..i+8 = E pairs p+1..p+4, carry into limb i+9
+        chain4(s.E[p + 1], s.E[p + 2], s.E[p + 3], s.E[p + 4], s.CY[I + 1], a, b[1], b[3], b[5], b[7]);
     }
 }
 
@@ -96,58 +106,30 @@ __device__ __forceinline__ void tile_mac(DiagAcc &s, const uint32_t (&a)[8], con
     tile_row<7>(s, a[7], b);
 }
 
-// D[0..16] = E + (O << 1 limb) + (CY << 8 limbs).  Each asm block is a self-contained carry chain
-// (the condition code never has to survive between two asm statements).
+// D[0..16] = E + (O << 1 limb) + (CY << 8 limbs).
 __device__ __forceinline__ void diag_finish(const DiagAcc &s, uint32_t (&d)[17])
 {
-    uint32_t c1;
-    d[0] = s.E[0];
-    // limbs 1..8 = E[1..8] + O[0..7]
-    asm("add.cc.u32 %0, %9, %17;\n\t"
-        "addc.cc.u32 %1, %10, %18;\n\t"
-        "addc.cc.u32 %2, %11, %19;\n\t"
-        "addc.cc.u32 %3, %12, %20;\n\t"
-        "addc.cc.u32 %4, %13, %21;\n\t"
-        "addc.cc.u32 %5, %14, %22;\n\t"
-        "addc.cc.u32 %6, %15, %23;\n\t"
-        "addc.cc.u32 %7, %16, %24;\n\t"
-        "addc.u32 %8, 0, 0;"
-        : "=r"(d[1]), "=r"(d[2]), "=r"(d[3]), "=r"(d[4]), "=r"(d[5]), "=r"(d[6]), "=r"(d[7]),
-          "=r"(d[8]), "=r"(c1)
-        : "r"(s.E[1]), "r"(s.E[2]), "r"(s.E[3]), "r"(s.E[4]), "r"(s.E[5]), "r"(s.E[6]),
-          "r"(s.E[7]), "r"(s.E[8]), "r"(s.O[0]), "r"(s.O[1]), "r"(s.O[2]), "r"(s.O[3]),
-          "r"(s.O[4]), "r"(s.O[5]), "r"(s.O[6]), "r"(s.O[7]));
-    // limbs 9..16 = E[9..15] + O[8..13] + c1   (add.cc c1 + 0xffffffff recreates the carry)
-    asm("add.cc.u32 %0, %8, 0xffffffff;\n\t"
-        "addc.cc.u32 %0, %9, %16;\n\t"
-        "addc.cc.u32 %1, %10, %17;\n\t"
-        "addc.cc.u32 %2, %11, %18;\n\t"
-        "addc.cc.u32 %3, %12, %19;\n\t"
-        "addc.cc.u32 %4, %13, %20;\n\t"
-        "addc.cc.u32 %5, %14, %21;\n\t"
-        "addc.cc.u32 %6, %15, 0;\n\t"
-        "addc.u32 %7, 0, 0;"
-        : "=&r"(d[9]), "=r"(d[10]), "=r"(d[11]), "=r"(d[12]), "=r"(d[13]), "=r"(d[14]),
-          "=r"(d[15]), "=r"(d[16])
-        : "r"(c1), "r"(s.E[9]), "r"(s.E[10]), "r"(s.E[11]), "r"(s.E[12]), "r"(s.E[13]),
-          "r"(s.E[14]), "r"(s.E[15]), "r"(s.O[8]), "r"(s.O[9]), "r"(s.O[10]), "r"(s.O[11]),
-          "r"(s.O[12]), "r"(s.O[13]));
-    // limbs 8..16 += CY[0..8]
-    asm("add.cc.u32 %0, %0, %9;\n\t"
-        "addc.cc.u32 %1, %1, %10;\n\t"
-        "addc.cc.u32 %2, %2, %11;\n\t"
-        "addc.cc.u32 %3, %3, %12;\n\t"
-        "addc.cc.u32 %4, %4, %13;\n\t"
-        "addc.cc.u32 %5, %5, %14;\n\t"
-        "addc.cc.u32 %6, %6, %15;\n\t"
-        "addc.cc.u32 %7, %7, %16;\n\t"
-        "addc.u32 %8, %8, %17;"
-        : "+r"(d[8]), "+r"(d[9]), "+r"(d[10]), "+r"(d[11]), "+r"(d[12]), "+r"(d[13]),
-          "+r"(d[14]), "+r"(d[15]), "+r"(d[16])
-        : "r"(s.CY[0]), "r"(s.CY[1]), "r"(s.CY[2]), "r"(s.CY[3]), "r"(s.CY[4]), "r"(s.CY[5]),
-          "r"(s.CY[6]), "r"(s.CY[7]), "r"(s.CY[8]));
+    uint32_t e[16], o[14];
+#pragma unroll
+    for (int i = 0; i < 8; i++) { e[2 * i] = (uint32_t)s.E[i]; e[2 * i + 1] = (uint32_t)(s.E[i] >> 32); }
+#pragma unroll
+    for (int i = 0; i < 7; i++) { o[2 * i] = (uint32_t)s.O[i]; o[2 * i + 1] = (uint32_t)(s.O[i] >> 32); }
+    unsigned long long cy = 0;
+    d[0] = e[0];
+#pragma unroll
+    for (int i = 1; i <= 16; i++) {
+        cy += (unsigned long long)(i < 16 ? e[i] : 0u) + (i - 1 < 14 ? o[i - 1] : 0u) + (i >= 8 ? s.CY[i - 8] : 0u);
+        d[i] = (uint32_t)cy;
+        cy >>= 32;
+    }
 }
 
+// 8 limbs from shared memory at the 32-bit shared-window address `saddr` (16-byte aligned).
+__device__ __forceinline__ void load_tile(uint32_t (&x)[8], uint32_t saddr)
+{
+    asm("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x[0]), "=r"(x[1]), "=r"(x[2]), "=r"(x[3]) : "r"(saddr));
+    asm("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(x[4]), "=r"(x[5]), "=r"(x[6]), "=r"(x[7]) : "r"(saddr));
+}
 __device__ __forceinline__ void load_tile(uint32_t (&x)[8], const limb *p)
 {
     const uint4 lo = reinterpret_cast<const uint4 *>(p)[0];
@@ -166,47 +148,84 @@ struct MulScratch {
 
 // Phase 1: tile diagonals 0..Kd-1 of A (Na tiles) x Bp (Nb tiles) -> P (low 8 limbs of each
 // diagonal), HI, OV.  Operands must be 16-byte aligned and zero padded to whole tiles.
-// Diagonals are dealt in rounds of T: cyclically (thread t takes t, t+T, ...), which balances the
-// up-ramp / plateau / down-ramp length profile of a full product, or -- snake = true -- in
-// boustrophedon order (odd rounds reversed), which balances the single ramp of a truncated product.
+//
+// A diagonal is shared by a GROUP of C = 2^sh consecutive lanes (C >= 4): lane c of the group takes
+// tiles I = Ilo + c, Ilo + c + C, ... and the C partial 17-limb sums are added with a shuffle
+// butterfly.  Consecutive groups of a warp own consecutive diagonals, whose lengths differ by one
+// tile, so the trip counts of the 32 lanes of a warp differ by at most ceil(8 / C) -- the ramps of
+// the product no longer idle three lanes in four -- and a block has C times more threads than
+// diagonals per pass, which is what small products (config 1) need.  Diagonals are dealt in passes of
+// T / 4 (cyclically: the up-ramp / plateau / down-ramp profile of a full product balances over the
+// passes; snake = true reverses odd passes, which balances the single ramp of a truncated product).
+// A pass that has fewer diagonals left than groups widens its groups (up to a whole warp).
+__device__ __forceinline__ void add17(uint32_t (&d)[17], const uint32_t (&x)[17])
+{
+    unsigned long long cy = 0;
+#pragma unroll
+    for (int i = 0; i < 17; i++) {
+        cy += (unsigned long long)d[i] + x[i];
+        d[i] = (uint32_t)cy;
+        cy >>= 32;
+    }
+}
+
 template <int T>
 __device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Kd,
                                               limb *P, const MulScratch &ms, bool snake)
 {
-    for (int base = 0; base < Kd; base += T) {
-        const int j = (snake && ((base / T) & 1)) ? (T - 1 - (int)threadIdx.x) : (int)threadIdx.x;
-        const int K = base + j;
-        if (K >= Kd) continue;
-        const int Ilo = max(0, K - Nb + 1), Ihi = min(Na - 1, K);
+    constexpr int G0 = T / 4;                       // diagonals per full pass (4 lanes each)
+    int pass = 0;
+    for (int base = 0; base < Kd; base += G0, ++pass) {
+        const int ndiag = min(G0, Kd - base);
+        int sh = 2;
+        while (sh < 5 && (ndiag << (sh + 1)) <= T) ++sh;
+        const int C = 1 << sh;
+        const int g = (int)threadIdx.x >> sh, c = (int)threadIdx.x & (C - 1);
+        const bool act = g < ndiag;
+        const int K = base + ((snake && (pass & 1)) ? (ndiag - 1 - g) : g);
+        const int Ilo = max(0, K - Nb + 1), Ihi = act ? min(Na - 1, K) : -1;
         DiagAcc s;
         s.clear();
-        if (Ilo <= Ihi) {
-            uint32_t a[8], b[8];
-            const limb *pa = A + TILE * Ilo;
-            const limb *pb = Bp + TILE * (K - Ilo);
-            load_tile(a, pa);
-            load_tile(b, pb);
-            for (int I = Ilo; I < Ihi; ++I) {
-                uint32_t an[8], bn[8];
-                pa += TILE;
-                pb -= TILE;
-                load_tile(an, pa);
-                load_tile(bn, pb);
-                tile_mac(s, a, b);
-#pragma unroll
-                for (int jj = 0; jj < 8; jj++) { a[jj] = an[jj]; b[jj] = bn[jj]; }
+        int I = Ilo + c;
+        if (I <= Ihi) {
+            uint32_t a0[8], b0[8], a1[8], b1[8];
+            const int step = 4 * TILE * C;                  // bytes between a lane's consecutive tiles
+            uint32_t pa = (uint32_t)__cvta_generic_to_shared(A) + 4 * TILE * I;
+            uint32_t pb = (uint32_t)__cvta_generic_to_shared(Bp) + 4 * TILE * (K - I);
+            load_tile(a0, pa);
+            load_tile(b0, pb);
+            // two tiles per trip with ping-pong operand registers (no register copies)
+            for (; I + C <= Ihi; I += 2 * C) {
+                pa += step; pb -= step;
+                load_tile(a1, pa);
+                load_tile(b1, pb);
+                tile_mac(s, a0, b0);
+                if (I + 2 * C <= Ihi) {
+                    pa += step; pb -= step;
+                    load_tile(a0, pa);
+                    load_tile(b0, pb);
+                }
+                tile_mac(s, a1, b1);
             }
-            tile_mac(s, a, b);
+            if (I <= Ihi) tile_mac(s, a0, b0);
         }
         uint32_t d[17];
         diag_finish(s, d);
-        uint4 *p4 = reinterpret_cast<uint4 *>(P + TILE * K);
-        uint4 *h4 = reinterpret_cast<uint4 *>(ms.HI + TILE * K);
-        p4[0] = make_uint4(d[0], d[1], d[2], d[3]);
-        p4[1] = make_uint4(d[4], d[5], d[6], d[7]);
-        h4[0] = make_uint4(d[8], d[9], d[10], d[11]);
-        h4[1] = make_uint4(d[12], d[13], d[14], d[15]);
-        ms.OV[K] = d[16];
+        for (int off = 1; off < C; off <<= 1) {
+            uint32_t x[17];
+#pragma unroll
+            for (int i = 0; i < 17; i++) x[i] = __shfl_xor_sync(0xffffffffu, d[i], off);
+            add17(d, x);
+        }
+        if (act && c == 0) {
+            uint4 *p4 = reinterpret_cast<uint4 *>(P + TILE * K);
+            uint4 *h4 = reinterpret_cast<uint4 *>(ms.HI + TILE * K);
+            p4[0] = make_uint4(d[0], d[1], d[2], d[3]);
+            p4[1] = make_uint4(d[4], d[5], d[6], d[7]);
+            h4[0] = make_uint4(d[8], d[9], d[10], d[11]);
+            h4[1] = make_uint4(d[12], d[13], d[14], d[15]);
+            ms.OV[K] = d[16];
+        }
     }
     __syncthreads();
 }

@@ -68,7 +68,7 @@ static MulLayout mul_layout(int a_limbs, int b_limbs, int c_limbs)
 }
 
 template <int T>
-__global__ void __launch_bounds__(T)
+__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
 mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b, int b_limbs,
              limb *__restrict__ c, int c_limbs, int batch, MulLayout L)
 {
@@ -168,12 +168,15 @@ bool device_props()
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-// threads per block for a number of `limbs` limbs: one thread per 16 limbs, 64..512
+// threads per block for numbers of `limbs` limbs.  Four lanes share a tile diagonal (mp_mul.cuh), so
+// a block of T threads covers T/4 diagonals = 2T limbs of product per pass.  256 threads at 128
+// registers let two blocks share an SM up to 4096 limbs; above that one block of 512 fills the SM.
 int threads_for(int limbs)
 {
-    int t = 64;
-    while (t < 512 && t * 16 < limbs) t *= 2;
-    return t;
+    if (limbs <= 128) return 64;
+    if (limbs <= 512) return 128;
+    if (limbs <= 4096) return 256;
+    return 512;
 }
 
 template <class K>
@@ -214,7 +217,7 @@ int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, 
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     const int big = a_limbs > b_limbs ? a_limbs : b_limbs;
-    switch (threads_for(2 * big)) {
+    switch (threads_for(big)) {
         case 64: return launch_mul<64>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
         case 128: return launch_mul<128>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);
         case 256: return launch_mul<256>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);

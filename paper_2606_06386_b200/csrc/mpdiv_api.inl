@@ -53,7 +53,7 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
 // shinv_batch kernel
 // ---------------------------------------------------------------------------------------
 template <int T>
-__global__ void __launch_bounds__(T)
+__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
 shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
              DivLayout L)
 {
@@ -93,7 +93,7 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // mpdiv_batch kernel: Alg. 3, one division per block
 // ---------------------------------------------------------------------------------------
 template <int T>
-__global__ void __launch_bounds__(T)
+__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L)
 {
