@@ -203,6 +203,9 @@ def per_config_table(binding, flush, peak_products: float):
         q = torch.empty_like(du)
         r = torch.empty_like(dv)
         t_div = float(np.median(time_steps(lambda: binding.mpdiv_batch(du, dv, q, r), 25, 3, flush)))
+        t_div_printed = float(np.median(time_steps(
+            lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED), 25, 3, flush)))
+        executed = executed_products(binding, du, dv, q, r)
         # R1 unit: M x M -> low M limbs (the paper's "full multiplication", M^2/2 limb products)
         a1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 0), b, m))
         b1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 1), b, m))
@@ -226,13 +229,28 @@ def per_config_table(binding, flush, peak_products: float):
             "mul_MxM_lowM_products_per_s": b * (m * (m + 1) / 2) / (t_m1 * 1e-3),
             "mul_nxn_full_products_per_s": b * nn * nn / (t_m2 * 1e-3),
             "hbm_GBps_div_io": b * 4 * (2 * m + 2 * n) / (t_div * 1e-3) / 1e9,
+            "printed_variant_div_ms": t_div_printed, "printed_variant_div_per_s": b / (t_div_printed * 1e-3),
+            "printed_variant_R1": t_div_printed / t_m1,
+            "executed_limb_products_per_division": executed / b,
+            "pipe_frac_executed": executed / (t_div * 1e-3) / peak_products,
         }
         if cfg != 5:
             row["W_limb_products"] = W_LIMB_PRODUCTS[m]
             row["roofline_frac"] = row["div_per_s"] * W_LIMB_PRODUCTS[m] / peak_products
+            row["printed_variant_roofline_frac"] = row["printed_variant_div_per_s"] * W_LIMB_PRODUCTS[m] / peak_products
         table["config%d" % cfg] = row
         del du, dv, q, r, a1, b1, c1, a2, b2, c2, w
     return table
+
+
+def executed_products(binding, du, dv, q, r, variant=None) -> int:
+    """Limb products one launch really issues (8x8 tiles counted by the kernel x 64, tile padding included)."""
+    import torch
+
+    binding.debug_counters(reset=True)
+    binding.mpdiv_batch(du, dv, q, r, variant=variant)
+    torch.cuda.synchronize()
+    return 64 * binding.debug_counters(reset=True)["tiles"]
 
 
 def run_ours(args):
@@ -309,7 +327,17 @@ def run_ours(args):
     roofline = None
     if cfg != 5:
         achieved = b * W_LIMB_PRODUCTS[m] / (kernel_ms * 1e-3)
+        executed = executed_products(binding, du, dv, q, r)
+        ms_printed = float(np.mean(time_steps(
+            lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED), args.steps, args.warmup, flush)))
         roofline = {
+            "note": "achieved = W(M) x batch / t with W(M) the limb products of the method AS PRINTED (SURVEY 8(d)); the "
+                    "default (clipped) variant skips the low part of w*x and u*shinv, the low and high parts of v'w and the "
+                    "high part of v*q (PAPER.md:507, :542), so frac may exceed 1; pipe_frac counts what really ran",
+            "executed_limb_products_per_launch": executed,
+            "pipe_frac": executed / (kernel_ms * 1e-3) / peak_products,
+            "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
+                                "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
             "bound": "alu", "kernel": "mpdiv_kernel",
             "achieved": achieved / 1e9, "peak": peak_products / 1e9, "unit": "G limb-products/s",
             "frac": achieved / peak_products, "traffic": None,

@@ -59,6 +59,23 @@ int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                 uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
 
 /*
+ * Variants of the method; both return the same exact (q, r).
+ *   MPDIV_VARIANT_PRINTED  Alg. 1-3 as printed: full products w*x, u*shinv, v*q and the close product
+ *                          v'w mod B^L.  Needs the 2M-limb product on chip:
+ *                          strides with u_limbs + v_limbs > 12288 return MPDIV_ERR_UNSUPPORTED.
+ *   MPDIV_VARIANT_CLIPPED  the paper's first future-work item: every product
+ *                          computes only the limb range the step keeps (top of w*x and u*shinv, middle
+ *                          of v'w, bottom of v*q); the +-1 correction of Alg. 3 becomes two bounded
+ *                          loops.  About 0.4 M^2 instead of 1.8 M^2 limb products per division.
+ * mpdiv_batch / shinv_batch use MPDIV_VARIANT_DEFAULT.
+ */
+#define MPDIV_VARIANT_PRINTED 0
+#define MPDIV_VARIANT_CLIPPED 1
+#define MPDIV_VARIANT_DEFAULT MPDIV_VARIANT_CLIPPED
+int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
+                   uint32_t *q, uint32_t *r, int batch, int variant, mpdiv_stream_t stream);
+
+/*
  * Multiplication, the unit of the paper's cost model (PAPER.md:105-106 MULT / MULTMOD, :166, :186):
  *     c_i = (a_i * b_i) mod B^c_limbs
  *   a : batch x a_limbs, b : batch x b_limbs (device, read);  c : batch x c_limbs (device, written)
@@ -71,12 +88,16 @@ int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs,
 /*
  * Whole shifted inverse as the division uses it, Alg. 1-2 and Theorem 2
  * (PAPER.md:160):   w_i = floor(B^h / v_i) + lambda_i,  lambda_i in {0, 1}
+ * (lambda in {-1, 0, 1} for the clipped variant)
  * i.e. the UNCORRECTED Newton result, so that its time is the "2..4 multiplications" of the cost
  * model.   v : batch x v_limbs (device, read);  w : batch x w_limbs (device, written),
  * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_LIMBS.  v_i = 0 gives w_i = all ones (counted as an error).
  */
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
                 int batch, mpdiv_stream_t stream);
+/* Same with an explicit variant; the clipped variant returns floor(B^h / v) + lambda, lambda in {-1, 0, 1}. */
+int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
+                   int batch, int variant, mpdiv_stream_t stream);
 
 /*
  * Host-buffer form of mpdiv_batch for end-to-end use: u, v, q, r are HOST pointers (pinned memory
@@ -102,15 +123,20 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
 
 /*
  * Debug counters accumulated by every mpdiv_batch / shinv_batch launch since the last reset
- * (device-side atomics on a library-owned 64-byte buffer; reading them synchronises `stream`):
- *   out[0] instances with the delta = -1 correction (u < v*q0)
- *   out[1] instances with one delta = +1 correction
- *   out[2] instances needing more than one +1 step (outside Theorem 2's range; expected 0)
+ * (device-side atomics on a library-owned 128-byte buffer; reading them synchronises `stream`):
+ *   out[0] instances with exactly one delta = -1 correction (u < v*q0)
+ *   out[1] instances with exactly one delta = +1 correction
+ *   out[2] instances needing more than one +1 step (printed variant: outside Theorem 2, expected 0;
+ *          clipped variant: allowed, the clipped quotient estimate may be one lower)
  *   out[3] one-limb divisors      out[4] u < v early exits      out[5] v = 0 instances
  *   out[6] Newton steps that took the negative branch of PowDiff (sign = 0)
  *   out[7] divisors that are an exact power of B (Alg. 1 line 9)
+ *   out[8] 8x8-limb tile products executed (x 64 = limb products issued, tile padding included)
+ *   out[9] instances needing more than one -1 step      out[10] instances whose correction loops hit
+ *          their bound of 8 (result not exact; expected 0)      out[11] Newton steps that ran clipped
+ *   out[12..15] reserved (0)
  */
-int mpdiv_debug_counters(unsigned long long out[8], int reset, mpdiv_stream_t stream);
+int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream);
 
 /* "mpdiv <version> sm_100a ..." */
 const char *mpdiv_version(void);

@@ -18,6 +18,8 @@ _LIB = None
 _VOIDP = ctypes.c_void_p
 
 OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
+VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
+VARIANT_DEFAULT = VARIANT_CLIPPED
 MAX_LIMBS = 8192
 
 
@@ -38,6 +40,8 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(path)
         i, sz = ctypes.c_int, ctypes.c_size_t
         L.mpdiv_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
+        L.mpdiv_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, i, _VOIDP]
+        L.shinv_batch_ex.argtypes = [_VOIDP, i, i, _VOIDP, i, i, i, _VOIDP]
         L.mpmul_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, _VOIDP]
         L.shinv_batch.argtypes = [_VOIDP, i, i, _VOIDP, i, i, _VOIDP]
         L.mpdiv_host_workspace_bytes.argtypes = [i, i, i]
@@ -49,14 +53,14 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_version.restype = ctypes.c_char_p
         L.mpdiv_strerror.argtypes = [i]
         L.mpdiv_strerror.restype = ctypes.c_char_p
-        for name in ("mpdiv_batch", "mpmul_batch", "shinv_batch", "mpdiv_batch_host",
+        for name in ("mpdiv_batch", "mpdiv_batch_ex", "shinv_batch_ex", "mpmul_batch", "shinv_batch", "mpdiv_batch_host",
                      "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_debug_counters"):
             getattr(L, name).restype = i
         _LIB = L
     return _LIB
 
 
-EXPORTS = ("mpdiv_batch", "mpmul_batch", "shinv_batch", "mpdiv_host_workspace_bytes",
+EXPORTS = ("mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
            "mpdiv_debug_counters", "mpdiv_version", "mpdiv_strerror")
 
@@ -89,8 +93,9 @@ def _raise(code: int, what: str):
 
 
 def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
-                r: torch.Tensor | None = None, stream=None):
-    """q = floor(u / v), r = u - q*v per row.  q has u's shape, r has v's shape."""
+                r: torch.Tensor | None = None, stream=None, variant: int | None = None):
+    """q = floor(u / v), r = u - q*v per row.  q has u's shape, r has v's shape.
+    variant: None -> mpdiv_batch (the library default), else mpdiv_batch_ex with that variant."""
     _check_dev(u, "u")
     _check_dev(v, "v")
     batch, ul = u.shape
@@ -105,8 +110,12 @@ def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
     _check_dev(r, "r")
     if tuple(q.shape) != (batch, ul) or tuple(r.shape) != (batch, vl):
         raise ValueError("q must be (batch, u_limbs) and r (batch, v_limbs)")
-    _raise(lib().mpdiv_batch(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
-                             _stream_ptr(stream)), "mpdiv_batch")
+    if variant is None:
+        _raise(lib().mpdiv_batch(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
+                                 _stream_ptr(stream)), "mpdiv_batch")
+    else:
+        _raise(lib().mpdiv_batch_ex(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
+                                    int(variant), _stream_ptr(stream)), "mpdiv_batch_ex")
     return q, r
 
 
@@ -125,15 +134,20 @@ def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor 
     return c
 
 
-def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = None, stream=None):
+def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = None, stream=None,
+                variant: int | None = None):
     """w = floor(B^h / v) + lambda, lambda in {0, 1}, per row (the uncorrected Newton result)."""
     _check_dev(v, "v")
     batch = v.shape[0]
     if w is None:
         w = torch.empty((batch, w_limbs), dtype=v.dtype, device=v.device)
     _check_dev(w, "w")
-    _raise(lib().shinv_batch(v.data_ptr(), v.shape[1], int(h), w.data_ptr(), w_limbs, batch,
-                             _stream_ptr(stream)), "shinv_batch")
+    if variant is None:
+        _raise(lib().shinv_batch(v.data_ptr(), v.shape[1], int(h), w.data_ptr(), w_limbs, batch,
+                                 _stream_ptr(stream)), "shinv_batch")
+    else:
+        _raise(lib().shinv_batch_ex(v.data_ptr(), v.shape[1], int(h), w.data_ptr(), w_limbs, batch, int(variant),
+                                    _stream_ptr(stream)), "shinv_batch_ex")
     return w
 
 
@@ -171,10 +185,11 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
     return int(prod.value), sink
 
 
-COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b")
+COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
+                 "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "rsv12", "rsv13", "rsv14", "rsv15")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:
-    out = (ctypes.c_ulonglong * 8)()
+    out = (ctypes.c_ulonglong * 16)()
     _raise(lib().mpdiv_debug_counters(out, 1 if reset else 0, _stream_ptr(stream)), "mpdiv_debug_counters")
     return {k: int(out[i]) for i, k in enumerate(COUNTER_NAMES)}

@@ -32,6 +32,7 @@ struct BlkScratch {
 struct Blk {
     BlkScratch *sc;
     uint32_t parity;   // which half of sc->code the next collective uses
+    uint32_t tiles;    // 8x8-limb tile products this thread has executed (debug counter)
 };
 
 // ---------------------------------------------------------------------------------------

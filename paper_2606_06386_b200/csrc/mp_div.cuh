@@ -10,15 +10,36 @@
 //     stays 16-byte aligned in shared memory; a longer prefix is always admissible.
 //   * one-limb divisors (Alg. 1 l.6 "divide by 1 digit") are mapped to two-limb ones:
 //     floor(B^h / v) = floor(B^(h+1) / (v*B)), and (u*B) div (v*B) = u div v with remainder r*B.
+//
+// Variants.  MPDIV_VARIANT_PRINTED runs Alg. 1-3 as printed: full products w*x, u*shinv, v*q and the
+// close product v'w mod B^L.  MPDIV_VARIANT_CLIPPED (default) is the paper's first future-work item
+// (clipped products): every product computes only the tile
+// diagonals whose limbs the step keeps --
+//   * v'w : columns [c, L) only, c = 8*(floor((c_x - 9)/8) - 1), c_x = d + 1 - prec(w) the lowest limb
+//           of x that can still move a kept limb of w*x;  x = P or ~P on those limbs (no borrow scan)
+//   * w*x : columns >= d + 1 - 9 only (the shift drops d + 1 limbs)
+//   * u*shinv : columns >= h - 9 only;   v*q : columns < k + 3 only (|u - v q0| < 4v)
+// An omitted low part E satisfies 0 <= E < B^(8 Klo + 9) (mp_mul.cuh), i.e. less than one unit of the
+// lowest kept limb, so every iterate moves by a few units of its lowest GUARD limb, the shifted inverse
+// by at most one unit (lambda in {-1,0,1}) and the quotient estimate by at most 2; the correction of
+// Alg. 3 becomes two bounded loops (r < 0: q-1, r+v;  r >= v: q+1, r-v) and the result stays exact.
+// Iterations whose operands are too short for the window to clip anything run the printed code.
 #pragma once
 #include "mp_mul.cuh"
 
 namespace mpd {
 
 // debug counters (include/mpdiv.h: mpdiv_debug_counters)
-__device__ unsigned long long g_counters[8];
+__device__ unsigned long long g_counters[16];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
-       CNT_SIGN_NEG, CNT_POW_B };
+       CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS };
+
+__device__ __forceinline__ void count_tiles(Blk &blk)
+{
+    uint32_t t = __reduce_add_sync(0xffffffffu, blk.tiles);
+    if ((threadIdx.x & 31) == 0 && t != 0) atomicAdd(&g_counters[CNT_TILES], (unsigned long long)t);
+    blk.tiles = 0;
+}
 
 __device__ __forceinline__ void count(int which)
 {
@@ -49,7 +70,8 @@ struct ShinvBufs {
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T>
-__device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk)
+__device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
+                                           bool clip)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
     const MulScratch &ms = bufs.ms;
@@ -102,11 +124,13 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
         const int hp = k + l + m - s + g;                      // h' of Step
         const int hpp = hp - m;                                // h'' of PowDiff
         const int pw = top_prec(Wc, min(wlen, l + g + 2));
+        const int d = hp - 2 * m;                              // limbs of w*x that shift_{2m-h'} drops
 
         // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
         const int L = pv + pw - (l - g) + 1;
         bool positive;
         int xl;                                                // limbs of x (upper bound)
+        int c = 0;                                             // X holds x / B^c
         if (L >= hpp) {
             // no room to truncate: full product and a comparison with B^h''
             mul_full<T>(Vp, pv, Wc, pw, P, ms, blk);
@@ -121,32 +145,58 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                 lin_addsub<T, true>(X, round_up(xl, TILE), LimbView{P, pl, 0}, UnitView{hpp}, 0u, blk);
             }
         } else {
-            // close product: only the L low limbs of v'w (MULTMOD)
-            mul_low<T>(Vp, pv, Wc, pw, L, P, ms, blk);
-            positive = P[L - 1] != 0u;                         // top limb set: v'w just below B^h''
-            xl = L;
-            if (positive)
-                lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, xl}, ZeroView{}, 1u, blk);
-            else
-                lin_copy<T>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
+            // c_x: x must be right down to limb c_x for w*x to be right down to limb d + 1
+            const int cx = d + 1 - pw;
+            const int Klo2 = (clip && cx >= 25) ? (cx - 9) / 8 - 1 : 0;
+            if (Klo2 <= 0) {
+                // close product: only the L low limbs of v'w (MULTMOD)
+                mul_low<T>(Vp, pv, Wc, pw, L, P, ms, blk);
+                positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
+                xl = L;
+                if (positive)
+                    lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, xl}, ZeroView{}, 1u, blk);
+                else
+                    lin_copy<T>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
+            } else {
+                // clipped close product: limbs [c, L) of v'w only; X holds x / B^c (low limbs taken as 0)
+                c = TILE * Klo2;
+                count(CNT_CLIPPED_STEPS);
+                mul_range<T>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
+                xl = L - c;
+                positive = P[xl - 1] != 0u;
+                for (int i = threadIdx.x; i < round_up(xl, TILE); i += T)
+                    X[i] = (i < xl) ? (positive ? ~P[i] : P[i]) : 0u;
+                __syncthreads();
+            }
         }
         if (!positive) count(CNT_SIGN_NEG);
         xl = top_prec(X, xl);
 
         // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
-        const int d = hp - 2 * m;                              // limbs of w*x that the shift drops
         const int nlen = round_up(l + m + g + 2, TILE);
         if (xl == 0) {
             lin_copy<T>(Wn, nlen, Wc, wlen, 1 - m);
         } else {
-            mul_full<T>(Wc, pw, X, xl, P, ms, blk);
-            const int tl = round_up(pw, TILE) + round_up(xl, TILE);
-            if (positive) {
-                lin_addsub<T, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, 1 + d}, 0u, blk);
+            // w*x / B^(d+1): the shift_{2m-h'} of Step and the shift_{-1} of Refine drop d + 1 limbs
+            const int dd = d + 1 - c;
+            const int Klo1 = (clip && dd >= 17) ? (dd - 9) / TILE : 0;
+            int tl, off;
+            if (Klo1 == 0) {
+                mul_full<T>(Wc, pw, X, xl, P, ms, blk);
+                tl = round_up(pw, TILE) + round_up(xl, TILE);
+                off = dd;
             } else {
-                // floor of a negative: borrow one when any dropped limb (0..d) of w*x is non-zero
-                const uint32_t bin = any_nonzero<T>(P, 0, min(d + 1, tl)) ? 1u : 0u;
-                lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, 1 + d}, bin, blk);
+                tl = mul_range<T>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
+                off = dd - TILE * Klo1;
+            }
+            if (positive) {
+                lin_addsub<T, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, 0u, blk);
+            } else {
+                // floor of a negative: borrow one when any dropped limb of w*x is non-zero (exact path only;
+                // a clipped step is off by less than a guard-limb unit either way)
+                uint32_t bin = 0u;
+                if (Klo1 == 0 && c == 0) bin = any_nonzero<T>(P, 0, min(dd, tl)) ? 1u : 0u;
+                lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
             }
         }
         l = l + m - 1;

@@ -170,12 +170,13 @@ __device__ __forceinline__ void add17(uint32_t (&d)[17], const uint32_t (&x)[17]
 }
 
 template <int T>
-__device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Kd,
-                                              limb *P, const MulScratch &ms, bool snake)
+__device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                              limb *P, const MulScratch &ms, bool snake, Blk &blk)
 {
     constexpr int G0 = T / 4;                       // diagonals per full pass (4 lanes each)
     int pass = 0;
-    for (int base = 0; base < Kd; base += G0, ++pass) {
+    uint32_t tiles = 0;
+    for (int base = Klo; base < Kd; base += G0, ++pass) {
         const int ndiag = min(G0, Kd - base);
         int sh = 2;
         while (sh < 5 && (ndiag << (sh + 1)) <= T) ++sh;
@@ -188,6 +189,7 @@ __device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp
         s.clear();
         int I = Ilo + c;
         if (I <= Ihi) {
+            tiles += (uint32_t)(Ihi - I) / (uint32_t)C + 1u;
             uint32_t a0[8], b0[8], a1[8], b1[8];
             const int step = 4 * TILE * C;                  // bytes between a lane's consecutive tiles
             uint32_t pa = (uint32_t)__cvta_generic_to_shared(A) + 4 * TILE * I;
@@ -227,16 +229,18 @@ __device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp
             ms.OV[K] = d[16];
         }
     }
+    blk.tiles += tiles;
     __syncthreads();
 }
 
-// Phase 2: resolve column blocks 0..Kc-1 in place: P[K] = P[K] + HI[K-1] + OV[K-2] + carries,
-// where diagonals >= Kd contribute nothing.  Kc <= Kd + 2.  Ends with __syncthreads.
+// Phase 2: resolve column blocks Klo..Kc-1 in place: P[K] = P[K] + HI[K-1] + OV[K-2] + carries,
+// where only diagonals Klo <= K < Kd contribute (nothing enters from below column block Klo).
+// Kc <= Kd + 2.  Ends with __syncthreads.
 template <int T>
-__device__ __noinline__ void mul_resolve(limb *P, int Kd, int Kc, const MulScratch &ms, Blk &blk)
+__device__ __noinline__ void mul_resolve(limb *P, int Klo, int Kd, int Kc, const MulScratch &ms, Blk &blk)
 {
     uint32_t cin = 0;
-    for (int base = 0; base < Kc; base += T) {
+    for (int base = Klo; base < Kc; base += T) {
         const int K = base + (int)threadIdx.x;
         const bool active = K < Kc;
         limb s[8];
@@ -248,12 +252,12 @@ __device__ __noinline__ void mul_resolve(limb *P, int Kd, int Kc, const MulScrat
 #pragma unroll
                 for (int j = 0; j < 8; j++) lo[j] = 0;
             }
-            if (K >= 1 && K - 1 < Kd) load_tile(hi, ms.HI + TILE * (K - 1));
+            if (K > Klo && K - 1 < Kd) load_tile(hi, ms.HI + TILE * (K - 1));
             else {
 #pragma unroll
                 for (int j = 0; j < 8; j++) hi[j] = 0;
             }
-            const uint32_t ov = (K >= 2 && K - 2 < Kd) ? ms.OV[K - 2] : 0u;
+            const uint32_t ov = (K - 2 >= Klo && K - 2 < Kd) ? ms.OV[K - 2] : 0u;
             c3 = add8(s, lo, hi);
             c3 += inc8(s, ov);
             ms.C3[K] = c3;
@@ -261,7 +265,7 @@ __device__ __noinline__ void mul_resolve(limb *P, int Kd, int Kc, const MulScrat
         __syncthreads();
         uint32_t g = 0, p = 0;
         if (active) {
-            const uint32_t cprev = (K >= 1) ? ms.C3[K - 1] : 0u;
+            const uint32_t cprev = (K > Klo) ? ms.C3[K - 1] : 0u;
             g = inc8(s, cprev);
             p = all_eq8(s, 0xffffffffu);
         }
@@ -288,8 +292,8 @@ __device__ __forceinline__ void mul_full(const limb *A, int na, const limb *Bp, 
 {
     const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
     const int Kd = Na + Nb - 1;
-    mul_diagonals<T>(A, Na, Bp, Nb, Kd, P, ms, false);
-    mul_resolve<T>(P, Kd, Na + Nb, ms, blk);
+    mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms, false, blk);
+    mul_resolve<T>(P, 0, Kd, Na + Nb, ms, blk);
 }
 
 template <int T>
@@ -300,8 +304,31 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
     const int Kfull = Na + Nb;
     const int Kc = min((L + TILE - 1) / TILE, Kfull);
     const int Kd = min(Kc, Kfull - 1);
-    mul_diagonals<T>(A, Na, Bp, Nb, Kd, P, ms, Kd < Kfull - 1);
-    mul_resolve<T>(P, Kd, Kc, ms, blk);
+    mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms, Kd < Kfull - 1, blk);
+    mul_resolve<T>(P, 0, Kd, Kc, ms, blk);
+}
+
+// Clipped ("range") product: only tile diagonals Klo <= K < Khi are computed, so the result is
+//     ((A * Bp) - E) mod B^(8*Khi),   0 <= E < B^(8*Klo + 9)
+// (E = the omitted low diagonals: column i+j = t holds at most t+1 products < B^2, and the omitted
+// columns end at 8*Klo + 6).  The block stores limb 8*Klo + i of that value at P[i] -- the buffers
+// only need 8*(Khi - Klo) limbs -- and limbs below 8*Klo are not produced.  Khi is clamped to the
+// size of the full product.  Returns the number of limbs stored.
+template <int T>
+__device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, int nb, int Klo, int Khi,
+                                         limb *P, const MulScratch &ms, Blk &blk)
+{
+    const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
+    const int Kfull = Na + Nb;
+    const int Kc = min(Khi, Kfull);
+    const int Kd = min(Kc, Kfull - 1);
+    MulScratch md;
+    md.HI = ms.HI - TILE * Klo;
+    md.OV = ms.OV - Klo;
+    md.C3 = ms.C3 - Klo;
+    mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, P - TILE * Klo, md, true, blk);
+    mul_resolve<T>(P - TILE * Klo, Klo, Kd, Kc, md, blk);
+    return TILE * max(Kc - Klo, 0);
 }
 
 }  // namespace mpd

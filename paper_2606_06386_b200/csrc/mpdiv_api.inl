@@ -13,15 +13,22 @@ struct DivLayout {
 };
 
 // M: limbs of the dividend side (u stride, or h for shinv_batch); n: divisor stride;
-// with_quotient: reserve the 2M-limb product of u * shinv.
-static DivLayout div_layout(int M, int n, bool with_quotient)
+// with_quotient: reserve the product scratch of u * shinv and v * q; clip: MPDIV_VARIANT_CLIPPED, whose
+// products only store the limbs they keep (about M/2 in Refine, M in the quotient phase).
+static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
 {
     DivLayout L;
     const int Mp = round_up(M, TILE);
     const int np = round_up(n, TILE);
-    L.x_words = np + 48;
-    L.p_words_r = Mp + 48;
-    L.p_words_q = with_quotient ? 2 * Mp + 32 : 0;
+    if (clip) {
+        L.x_words = round_up(Mp / 2 + 96, TILE);
+        L.p_words_r = round_up(Mp / 2 + 160, TILE);
+        L.p_words_q = with_quotient ? (Mp > np ? Mp : np) + 64 : 0;
+    } else {
+        L.x_words = np + 48;
+        L.p_words_r = Mp + 48;
+        L.p_words_q = with_quotient ? 2 * Mp + 32 : 0;
+    }
     const int ovr = round_up(L.p_words_r / TILE, 4), ovq = round_up(L.p_words_q / TILE, 4);
     const int big_r = L.x_words + 2 * L.p_words_r + 2 * ovr;
     const int big_q = 2 * L.p_words_q + 2 * ovq;
@@ -55,7 +62,7 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
 template <int T>
 __global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
 shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
-             DivLayout L)
+             DivLayout L, int clip)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     limb *V = smem + L.v_off;
@@ -80,13 +87,14 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
             count(CNT_ONE_LIMB);
             if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }   // v*B at the (aligned) base V
             __syncthreads();
-            nw = shinv_block<T>(V, 1, h + 1, bufs, blk);
+            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0);
         } else {
-            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk);
+            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0);
         }
         store_number<T>(wout, bufs.WA, w_limbs, round_up(nw, TILE));
         __syncthreads();
     }
+    count_tiles(blk);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -95,7 +103,7 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 template <int T>
 __global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
-             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L)
+             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
@@ -152,7 +160,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk);
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0);
         const int psh = top_prec(WA, nw);
 
         // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
@@ -165,38 +173,72 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
         __syncthreads();
 
-        // a9: q0 = shift_{-h}(u * shinv)  (Alg. 3 line 2); the full product, as printed
         const int nq = h - k + 1;                          // q0 <= B^(h-k): at most h-k+1 limbs
         const int qlen = round_up(nq + 1, TILE);
         limb *Q = WA;
-        if (psh == 0) {
-            lin_zero<T>(Q, qlen);
-        } else {
-            mul_full<T>(Ub, h, WA, psh, PQ, mq, blk);
-            const int pl = round_up(h, TILE) + round_up(psh, TILE);
-            lin_copy<T>(Q, qlen, PQ, pl, h);               // WA (shinv) is dead: reuse it for q
-        }
-        const int pq = top_prec(Q, nq);
-
-        // a10: p = v * q0  (Alg. 3 line 3)
-        const int rlen = round_up(h + 1, TILE);            // p <= u + v < 2 B^h
-        int pl = 0;
-        if (pq > 0) {
-            mul_full<T>(Vb, k + 1, Q, pq, PQ, mq, blk);
-            pl = round_up(k + 1, TILE) + round_up(pq, TILE);
-        }
-
-        // a11: corrections (Alg. 3 lines 4-10, Theorem 2)
         limb *R = PQ, *R2 = mq.HI;                         // r in place over p; HI is free after the product
-        uint32_t borrow = lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
-        if (borrow) {                                      // u < v*q0: delta = -1
-            count(CNT_DELTA_NEG);
-            lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
-            lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+        int rlen;                                          // limbs of the remainder arithmetic
+        int minus = 0;
+        if (!clip) {
+            // a9: q0 = shift_{-h}(u * shinv)  (Alg. 3 line 2); the full product, as printed
+            if (psh == 0) {
+                lin_zero<T>(Q, qlen);
+            } else {
+                mul_full<T>(Ub, h, WA, psh, PQ, mq, blk);
+                const int pl = round_up(h, TILE) + round_up(psh, TILE);
+                lin_copy<T>(Q, qlen, PQ, pl, h);           // WA (shinv) is dead: reuse it for q
+            }
+            const int pq = top_prec(Q, nq);
+
+            // a10: p = v * q0  (Alg. 3 line 3)
+            rlen = round_up(h + 1, TILE);                  // p <= u + v < 2 B^h
+            int pl = 0;
+            if (pq > 0) {
+                mul_full<T>(Vb, k + 1, Q, pq, PQ, mq, blk);
+                pl = round_up(k + 1, TILE) + round_up(pq, TILE);
+            }
+
+            // a11: corrections (Alg. 3 lines 4-10, Theorem 2)
+            const uint32_t borrow =
+                lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
+            if (borrow) {                                  // u < v*q0: delta = -1
+                minus = 1;
+                lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
+                lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+            }
+        } else {
+            // a9 clipped: only the columns >= h - 9 of u * shinv; q0' in {q0 - 1, q0}
+            if (psh == 0) {
+                lin_zero<T>(Q, qlen);
+            } else {
+                const int Klo = (h >= 17) ? (h - 9) / TILE : 0;
+                const int pl = mul_range<T>(Ub, h, WA, psh, Klo, 1 << 20, PQ, mq, blk);
+                lin_copy<T>(Q, qlen, PQ, pl, h - TILE * Klo);
+            }
+            const int pq = top_prec(Q, nq);
+
+            // a10 clipped: |u - v q0'| < 4v < B^(k+2), so the remainder arithmetic runs mod B^rlen
+            rlen = round_up(k + 3, TILE);
+            int pl = 0;
+            if (pq > 0) {
+                mul_low<T>(Vb, k + 1, Q, pq, rlen, PQ, mq, blk);
+                pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
+            }
+
+            // a11: r = u - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
+            lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
+            while (R[rlen - 1] != 0u && minus < 8) {
+                ++minus;
+                lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
+                lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+            }
         }
+        if (minus == 1) count(CNT_DELTA_NEG);
+        if (minus > 1) count(CNT_DELTA_NEG_MULTI);
         int plus = 0;
-        for (int step = 0; step < 4; ++step) {             // r >= v: delta = +1 (at most once by Theorem 2)
-            borrow = lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
+        for (int step = 0; step < 8; ++step) {             // r >= v: delta = +1 (once by Theorem 2 as printed)
+            const uint32_t borrow =
+                lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
             if (borrow) break;
             limb *t = R; R = R2; R2 = t;
             lin_addsub<T, false>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
@@ -204,6 +246,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
         if (plus == 1) count(CNT_DELTA_POS);
         if (plus > 1) count(CNT_DELTA_MULTI);
+        if (plus >= 8 || minus >= 8) count(CNT_DELTA_OUT_OF_RANGE);
 
         // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
         store_number<T>(qg, Q, u_limbs, min(qlen, u_limbs));
@@ -211,6 +254,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         else store_number<T>(rg, R, v_limbs, min(k + 1, v_limbs));
         __syncthreads();
     }
+    count_tiles(blk);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -220,24 +264,24 @@ namespace {
 
 template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-               cudaStream_t st)
+               cudaStream_t st, int clip)
 {
-    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true);
+    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L);
+    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip);
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
 template <int T>
-int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st)
+int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st, int clip)
 {
-    const DivLayout L = div_layout(h + 1, v_limbs, false);
+    const DivLayout L = div_layout(h + 1, v_limbs, false, clip != 0);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(shinv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
-    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L);
+    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L, clip);
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
@@ -258,22 +302,38 @@ extern "C" {
 int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
                 int batch, mpdiv_stream_t stream)
 {
+    return mpdiv_batch_ex(u, u_limbs, v, v_limbs, q, r, batch, MPDIV_VARIANT_DEFAULT, stream);
+}
+
+int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
+                   int batch, int variant, mpdiv_stream_t stream)
+{
+    if (variant != MPDIV_VARIANT_PRINTED && variant != MPDIV_VARIANT_CLIPPED) return MPDIV_ERR_BAD_ARG;
+    const int clip = variant == MPDIV_VARIANT_CLIPPED;
     int rc = check_div_args(u, u_limbs, v, v_limbs, q, r, batch);
     if (rc != MPDIV_OK) return rc;
     if (!aligned16(u) || !aligned16(v) || !aligned16(q) || !aligned16(r)) return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     switch (threads_for(u_limbs)) {
-        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st);
-        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st);
-        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st);
-        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st);
+        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
+        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
+        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
+        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
     }
 }
 
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch,
                 mpdiv_stream_t stream)
 {
+    return shinv_batch_ex(v, v_limbs, h, w, w_limbs, batch, MPDIV_VARIANT_DEFAULT, stream);
+}
+
+int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch, int variant,
+                   mpdiv_stream_t stream)
+{
+    if (variant != MPDIV_VARIANT_PRINTED && variant != MPDIV_VARIANT_CLIPPED) return MPDIV_ERR_BAD_ARG;
+    const int clip = variant == MPDIV_VARIANT_CLIPPED;
     if (!v || !w || v_limbs <= 0 || w_limbs <= 0 || batch <= 0 || h < 1) return MPDIV_ERR_BAD_ARG;
     if ((v_limbs | w_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (w_limbs < h + 1) return MPDIV_ERR_BAD_ARG;
@@ -282,10 +342,10 @@ int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     switch (threads_for(h)) {
-        case 64: return launch_shinv<64>(v, v_limbs, h, w, w_limbs, batch, st);
-        case 128: return launch_shinv<128>(v, v_limbs, h, w, w_limbs, batch, st);
-        case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st);
-        default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st);
+        case 64: return launch_shinv<64>(v, v_limbs, h, w, w_limbs, batch, st, clip);
+        case 128: return launch_shinv<128>(v, v_limbs, h, w, w_limbs, batch, st, clip);
+        case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st, clip);
+        default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st, clip);
     }
 }
 
@@ -318,14 +378,14 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     return MPDIV_OK;
 }
 
-int mpdiv_debug_counters(unsigned long long out[8], int reset, mpdiv_stream_t stream)
+int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream)
 {
     if (!out) return MPDIV_ERR_BAD_ARG;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     if (cudaStreamSynchronize(st) != cudaSuccess) return MPDIV_ERR_CUDA;
-    if (cudaMemcpyFromSymbol(out, g_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(out, g_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
     if (reset) {
-        unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        unsigned long long z[16] = {0};
         if (cudaMemcpyToSymbol(g_counters, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
     }
     return MPDIV_OK;

@@ -27,14 +27,18 @@ def host(t: torch.Tensor) -> np.ndarray:
     return t.cpu().numpy().view(np.uint32)
 
 
-def gpu_div(u, v):
-    q, r = binding.mpdiv_batch(dev(u), dev(v))
+PRINTED, CLIPPED = binding.VARIANT_PRINTED, binding.VARIANT_CLIPPED
+VARIANTS = [pytest.param(CLIPPED, id="clipped"), pytest.param(PRINTED, id="printed")]
+
+
+def gpu_div(u, v, variant=None):
+    q, r = binding.mpdiv_batch(dev(u), dev(v), variant=variant)
     torch.cuda.synchronize()
     return host(q), host(r)
 
 
-def check_div(u, v, what=""):
-    q, r = gpu_div(u, v)
+def check_div(u, v, what="", variant=None):
+    q, r = gpu_div(u, v, variant)
     qo, ro = oracle.divmod_batch(u, v, threads=NCPU)
     bad = np.nonzero((q != qo).any(axis=1) | (r != ro).any(axis=1))[0]
     assert bad.size == 0, "%s: %d of %d instances differ, first %d" % (what, bad.size, u.shape[0], bad[0])
@@ -73,32 +77,35 @@ def test_mul_parity(an, bn, cn):
 # ------------------------------------------------------------------ shifted inverse
 @pytest.mark.parametrize("vn,h", [(4, 7), (8, 16), (16, 17), (64, 128), (512, 1024), (1024, 2048),
                                   (260, 777), (2048, 4096), (4096, 8192), (512, 512), (512, 300)])
-def test_shinv_parity(vn, h):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_shinv_parity(vn, h, variant):
     batch = 24
     wn = (h + 1 + 3) // 4 * 4
     _, v = inputs.directed(max(vn, 8), vn, count=batch, seed=inputs.SEED + h)
     v2 = inputs._uniform(inputs.rng_for(201, h % 65536), 8, vn)
     inputs._force_top_nonzero(v2)
     v = np.concatenate([v, v2])
-    w = host(binding.shinv_batch(dev(v), h, wn))
+    w = host(binding.shinv_batch(dev(v), h, wn, variant=variant))
     wo = oracle.shinv_batch(v, h, wn)
-    lam_hist = {0: 0, 1: 0}
+    allowed = (0, 1) if variant == PRINTED else (-1, 0, 1)      # Theorem 2; one more unit when clipped
+    lam_hist = {-1: 0, 0: 0, 1: 0}
     for i in range(v.shape[0]):
         lam = inputs.from_limbs(w[i]) - inputs.from_limbs(wo[i])
-        assert lam in (0, 1), "instance %d: lambda = %d (Theorem 2 allows 0 or 1)" % (i, lam)
+        assert lam in allowed, "instance %d: lambda = %d (allowed %s)" % (i, lam, allowed)
         lam_hist[lam] += 1
     print("lambda histogram", lam_hist)
 
 
 # ------------------------------------------------------------------ division: the five configs
+@pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
-def test_div_config_full_size(cfg):
+def test_div_config_full_size(cfg, variant):
     """BASELINE.json configs at full size, in the launch configuration bench.py times.
 
     Configs 1-2 and 5 are checked on every instance; 3 and 4 (oracle: tens of ms per division)
     on a seeded sample of instances, each compared limb by limb."""
     u, v = inputs.config(cfg)
-    q, r = gpu_div(u, v)
+    q, r = gpu_div(u, v, variant)
     batch = u.shape[0]
     if cfg in (3, 4):
         pick = np.sort(inputs.rng_for(300 + cfg).choice(batch, size=96 if cfg == 3 else 48, replace=False))
@@ -110,12 +117,13 @@ def test_div_config_full_size(cfg):
         cfg, bad.size, pick.size, pick[bad[0]])
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("cfg", [3, 4])
-def test_div_config_invariants_all_instances(cfg):
+def test_div_config_invariants_all_instances(cfg, variant):
     """Properties that hold at any size, on EVERY instance of the big configs:
     r < v limb-wise compare and u = q*v + r checked with Python integers (independent of both sides)."""
     u, v = inputs.config(cfg)
-    q, r = gpu_div(u, v)
+    q, r = gpu_div(u, v, variant)
     step = 1 if cfg == 3 else 1
     for i in range(0, u.shape[0], step):
         ui, vi = inputs.from_limbs(u[i]), inputs.from_limbs(v[i])
@@ -128,36 +136,54 @@ def test_div_config_invariants_all_instances(cfg):
                                        (128, 64, 512), (1024, 512, 768), (2048, 1024, 384),
                                        (2048, 2048, 384), (4096, 2048, 128), (8192, 4096, 48),
                                        (8192, 8192, 32), (1028, 516, 256), (100, 52, 256)])
-def test_div_directed(M, n, count):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_div_directed(M, n, count, variant):
+    if variant == PRINTED and M + n > 12288:
+        with pytest.raises(binding.MpdivError) as e:     # the 2M-limb product does not fit on chip
+            gpu_div(*inputs.directed(M, n, count=2), variant)
+        assert e.value.code == binding.ERR_UNSUPPORTED
+        return
     binding.debug_counters(reset=True)
     u, v = inputs.directed(M, n, count=count)
-    check_div(u, v, "directed M=%d n=%d" % (M, n))
+    check_div(u, v, "directed M=%d n=%d" % (M, n), variant)
     cnt = binding.debug_counters()
     print("counters", cnt)
-    assert cnt["delta_multi"] == 0, "a quotient needed more than one +1 step (Theorem 2 violated)"
+    assert cnt["delta_out_of_range"] == 0
+    if variant == PRINTED:
+        assert cnt["delta_multi"] == 0, "a quotient needed more than one +1 step (Theorem 2 violated)"
+        assert cnt["delta_neg_multi"] == 0 and cnt["clipped_steps"] == 0
 
 
-def test_directed_reaches_corner_paths():
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_directed_reaches_corner_paths(variant):
     """The directed set must actually drive the rare branches: delta = -1, delta = +1,
     the negative PowDiff sign, powers of B and one-limb divisors."""
     binding.debug_counters(reset=True)
     u, v = inputs.directed(64, 32, count=2048)
-    check_div(u, v, "directed 64/32")
+    check_div(u, v, "directed 64/32", variant)
+    u, v = inputs.directed(512, 256, count=1024)       # long enough for the clipped windows to bite
+    check_div(u, v, "directed 512/256", variant)
     cnt = binding.debug_counters(reset=True)
     print("counters", cnt)
-    for key in ("delta_neg", "delta_pos", "sign_neg", "pow_b", "one_limb", "u_lt_v"):
+    for key in ("delta_neg", "delta_pos", "sign_neg", "pow_b", "one_limb", "u_lt_v", "tiles"):
         assert cnt[key] > 0, "%s never fired" % key
-    assert cnt["delta_multi"] == 0
+    assert cnt["delta_out_of_range"] == 0
+    if variant == PRINTED:
+        assert cnt["delta_multi"] == 0 and cnt["clipped_steps"] == 0
+    else:
+        assert cnt["clipped_steps"] > 0
 
 
-@pytest.mark.parametrize("M", [64, 1024, 2048])
-def test_div_paper_shape(M):
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("M", [64, 1024, 2048, 8192])
+def test_div_paper_shape(M, variant):
     """The paper's own workload shape: prec(u) = M-2, prec(v) uniform in 2..M/2."""
-    u, v = inputs.paper_shape(256, M)
-    check_div(u, v, "paper shape M=%d" % M)
+    u, v = inputs.paper_shape(256 if M < 8192 else 48, M)
+    check_div(u, v, "paper shape M=%d" % M, variant)
 
 
-def test_div_random_effective_precisions():
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_div_random_effective_precisions(variant):
     """1000 randomised instances with random values and random effective precisions."""
     rng = inputs.rng_for(400)
     M = 256
@@ -167,7 +193,21 @@ def test_div_random_effective_precisions():
         lv = int(rng.integers(1, M + 1))
         us.append(inputs._random_int(rng, lu))
         vs.append(inputs._random_int(rng, lv))
-    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions")
+    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions", variant)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_div_random_effective_precisions_large(variant):
+    """Random effective precisions at the 2^16-bit stride: every clipping window position occurs."""
+    rng = inputs.rng_for(401)
+    M = 2048
+    us, vs = [], []
+    for _ in range(400):
+        lv = int(rng.integers(1, M + 1))
+        lu = int(rng.integers(0, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, lv))
+    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions 2048", variant)
 
 
 def test_div_zero_divisor_does_not_trap():
