@@ -34,6 +34,23 @@ __device__ unsigned long long g_counters[16];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
        CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS };
 
+// Phase timing for tuning builds only (-DMPDIV_PHASE_TIMING): thread 0 of block 0 accumulates the cycles
+// between consecutive PHASE() marks.  Compiles to nothing in the product build.
+#ifdef MPDIV_PHASE_TIMING
+__device__ unsigned long long g_phase[64];
+__device__ long long g_phase_t0;
+#define PHASE(i)                                                        \
+    do {                                                                \
+        if (blockIdx.x == 0 && threadIdx.x == 0) {                      \
+            const long long t_ = clock64();                             \
+            g_phase[(i)] += (unsigned long long)(t_ - g_phase_t0);      \
+            g_phase_t0 = t_;                                            \
+        }                                                               \
+    } while (0)
+#else
+#define PHASE(i) do { } while (0)
+#endif
+
 __device__ __forceinline__ void count_tiles(Blk &blk)
 {
     uint32_t t = __reduce_add_sync(0xffffffffu, blk.tiles);
@@ -115,6 +132,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     int wlen = TILE;                                           // valid (zero padded) words of Wc
 
     // ---- Refine (Alg. 1 lines 15-28) ------------------------------------------------------------
+    PHASE(0);
     for (int it = 0; it < iters; ++it) {
         const int m = min(H + 1 - l, l);
         int s = max(0, k - 2 * l + 1 - g);
@@ -171,6 +189,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
         }
         if (!positive) count(CNT_SIGN_NEG);
         xl = top_prec(X, xl);
+        PHASE(16 + (it & 15));
 
         // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
         const int nlen = round_up(l + m + g + 2, TILE);
@@ -199,6 +218,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                 lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
             }
         }
+        PHASE(32 + (it & 15));
         l = l + m - 1;
         wlen = nlen;
         limb *t = Wc; Wc = Wn; Wn = t;

@@ -170,9 +170,9 @@ __device__ __forceinline__ void add17(uint32_t (&d)[17], const uint32_t (&x)[17]
 }
 
 template <int T>
-__device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
-                                              limb *P, const MulScratch &ms, bool snake, Blk &blk)
-{
+__device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                                  limb *P, limb *HI, uint32_t *OV, bool snake)
+{   // everything by value: a reference argument of a noinline function lives in local memory
     constexpr int G0 = T / 4;                       // diagonals per full pass (4 lanes each)
     int pass = 0;
     uint32_t tiles = 0;
@@ -221,24 +221,25 @@ __device__ __noinline__ void mul_diagonals(const limb *A, int Na, const limb *Bp
         }
         if (act && c == 0) {
             uint4 *p4 = reinterpret_cast<uint4 *>(P + TILE * K);
-            uint4 *h4 = reinterpret_cast<uint4 *>(ms.HI + TILE * K);
+            uint4 *h4 = reinterpret_cast<uint4 *>(HI + TILE * K);
             p4[0] = make_uint4(d[0], d[1], d[2], d[3]);
             p4[1] = make_uint4(d[4], d[5], d[6], d[7]);
             h4[0] = make_uint4(d[8], d[9], d[10], d[11]);
             h4[1] = make_uint4(d[12], d[13], d[14], d[15]);
-            ms.OV[K] = d[16];
+            OV[K] = d[16];
         }
     }
-    blk.tiles += tiles;
     __syncthreads();
+    return tiles;
 }
 
 // Phase 2: resolve column blocks Klo..Kc-1 in place: P[K] = P[K] + HI[K-1] + OV[K-2] + carries,
 // where only diagonals Klo <= K < Kd contribute (nothing enters from below column block Klo).
 // Kc <= Kd + 2.  Ends with __syncthreads.
 template <int T>
-__device__ __noinline__ void mul_resolve(limb *P, int Klo, int Kd, int Kc, const MulScratch &ms, Blk &blk)
-{
+__device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, limb *HI, uint32_t *OV,
+                                                uint32_t *C3, Blk blk)
+{   // blk by value (registers); the advanced collective parity is returned
     uint32_t cin = 0;
     for (int base = Klo; base < Kc; base += T) {
         const int K = base + (int)threadIdx.x;
@@ -252,20 +253,20 @@ __device__ __noinline__ void mul_resolve(limb *P, int Klo, int Kd, int Kc, const
 #pragma unroll
                 for (int j = 0; j < 8; j++) lo[j] = 0;
             }
-            if (K > Klo && K - 1 < Kd) load_tile(hi, ms.HI + TILE * (K - 1));
+            if (K > Klo && K - 1 < Kd) load_tile(hi, HI + TILE * (K - 1));
             else {
 #pragma unroll
                 for (int j = 0; j < 8; j++) hi[j] = 0;
             }
-            const uint32_t ov = (K - 2 >= Klo && K - 2 < Kd) ? ms.OV[K - 2] : 0u;
+            const uint32_t ov = (K - 2 >= Klo && K - 2 < Kd) ? OV[K - 2] : 0u;
             c3 = add8(s, lo, hi);
             c3 += inc8(s, ov);
-            ms.C3[K] = c3;
+            C3[K] = c3;
         }
         __syncthreads();
         uint32_t g = 0, p = 0;
         if (active) {
-            const uint32_t cprev = (K > Klo) ? ms.C3[K - 1] : 0u;
+            const uint32_t cprev = (K > Klo) ? C3[K - 1] : 0u;
             g = inc8(s, cprev);
             p = all_eq8(s, 0xffffffffu);
         }
@@ -280,6 +281,7 @@ __device__ __noinline__ void mul_resolve(limb *P, int Klo, int Kd, int Kc, const
         cin = cout;
     }
     __syncthreads();
+    return blk.parity;
 }
 
 // P[0 .. 8*Kc) = (A * Bp) restricted to tile diagonals < Kd, carries resolved.
@@ -292,8 +294,8 @@ __device__ __forceinline__ void mul_full(const limb *A, int na, const limb *Bp, 
 {
     const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
     const int Kd = Na + Nb - 1;
-    mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms, false, blk);
-    mul_resolve<T>(P, 0, Kd, Na + Nb, ms, blk);
+    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, false);
+    blk.parity = mul_resolve<T>(P, 0, Kd, Na + Nb, ms.HI, ms.OV, ms.C3, blk);
 }
 
 template <int T>
@@ -304,8 +306,8 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
     const int Kfull = Na + Nb;
     const int Kc = min((L + TILE - 1) / TILE, Kfull);
     const int Kd = min(Kc, Kfull - 1);
-    mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms, Kd < Kfull - 1, blk);
-    mul_resolve<T>(P, 0, Kd, Kc, ms, blk);
+    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, Kd < Kfull - 1);
+    blk.parity = mul_resolve<T>(P, 0, Kd, Kc, ms.HI, ms.OV, ms.C3, blk);
 }
 
 // Clipped ("range") product: only tile diagonals Klo <= K < Khi are computed, so the result is
@@ -322,12 +324,10 @@ __device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, 
     const int Kfull = Na + Nb;
     const int Kc = min(Khi, Kfull);
     const int Kd = min(Kc, Kfull - 1);
-    MulScratch md;
-    md.HI = ms.HI - TILE * Klo;
-    md.OV = ms.OV - Klo;
-    md.C3 = ms.C3 - Klo;
-    mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, P - TILE * Klo, md, true, blk);
-    mul_resolve<T>(P - TILE * Klo, Klo, Kd, Kc, md, blk);
+    limb *Pd = P - TILE * Klo, *HId = ms.HI - TILE * Klo;
+    uint32_t *OVd = ms.OV - Klo, *C3d = ms.C3 - Klo;
+    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, true);
+    blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
     return TILE * max(Kc - Klo, 0);
 }
 

@@ -1,6 +1,7 @@
 // libmpdiv.so -- kernels and C ABI (include/mpdiv.h).  sm_100a only.
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cuda_runtime.h>
 
 #include "../../include/mpdiv.h"
@@ -68,7 +69,7 @@ static MulLayout mul_layout(int a_limbs, int b_limbs, int c_limbs)
 }
 
 template <int T>
-__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
+__global__ void __launch_bounds__(T, 512 / T)
 mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b, int b_limbs,
              limb *__restrict__ c, int c_limbs, int batch, MulLayout L)
 {
@@ -173,6 +174,10 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 // registers let two blocks share an SM up to 4096 limbs; above that one block of 512 fills the SM.
 int threads_for(int limbs)
 {
+    if (const char *e = getenv("MPDIV_THREADS")) {     // tuning experiments only
+        const int t = atoi(e);
+        if (t == 64 || t == 128 || t == 256 || t == 512) return t;
+    }
     if (limbs <= 128) return 64;
     if (limbs <= 512) return 128;
     if (limbs <= 4096) return 256;

@@ -60,7 +60,7 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
 // shinv_batch kernel
 // ---------------------------------------------------------------------------------------
 template <int T>
-__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
+__global__ void __launch_bounds__(T, 512 / T)
 shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
              DivLayout L, int clip)
 {
@@ -101,7 +101,7 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // mpdiv_batch kernel: Alg. 3, one division per block
 // ---------------------------------------------------------------------------------------
 template <int T>
-__global__ void __launch_bounds__(T, (T <= 256) ? 2 : 1)
+__global__ void __launch_bounds__(T, 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip)
 {
@@ -124,6 +124,9 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         limb *qg = q + (size_t)inst * u_limbs;
         limb *rg = r + (size_t)inst * v_limbs;
 
+#ifdef MPDIV_PHASE_TIMING
+        if (blockIdx.x == 0 && threadIdx.x == 0) g_phase_t0 = clock64();
+#endif
         // a1/a2: load, precisions ("h <- prec(u)")
         load_number<T>(V + 4, v + (size_t)inst * v_limbs, v_limbs, vpad - 4);
         load_number<T>(U + 4, ug, u_limbs, upad - 4);
@@ -160,8 +163,10 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
+        PHASE(1);
         const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0);
         const int psh = top_prec(WA, nw);
+        PHASE(2);
 
         // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
         if (one_limb) {
@@ -173,6 +178,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
         __syncthreads();
 
+        PHASE(3);
         const int nq = h - k + 1;                          // q0 <= B^(h-k): at most h-k+1 limbs
         const int qlen = round_up(nq + 1, TILE);
         limb *Q = WA;
@@ -216,6 +222,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 lin_copy<T>(Q, qlen, PQ, pl, h - TILE * Klo);
             }
             const int pq = top_prec(Q, nq);
+            PHASE(4);
 
             // a10 clipped: |u - v q0'| < 4v < B^(k+2), so the remainder arithmetic runs mod B^rlen
             rlen = round_up(k + 3, TILE);
@@ -225,6 +232,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
             }
 
+            PHASE(5);
             // a11: r = u - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
             lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
             while (R[rlen - 1] != 0u && minus < 8) {
@@ -247,12 +255,14 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         if (plus == 1) count(CNT_DELTA_POS);
         if (plus > 1) count(CNT_DELTA_MULTI);
         if (plus >= 8 || minus >= 8) count(CNT_DELTA_OUT_OF_RANGE);
+        PHASE(6);
 
         // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
         store_number<T>(qg, Q, u_limbs, min(qlen, u_limbs));
         if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
         else store_number<T>(rg, R, v_limbs, min(k + 1, v_limbs));
         __syncthreads();
+        PHASE(7);
     }
     count_tiles(blk);
 }
@@ -377,6 +387,19 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     if (cudaMemcpyAsync(r_host, dr, vb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MPDIV_ERR_CUDA;
     return MPDIV_OK;
 }
+
+#ifdef MPDIV_PHASE_TIMING
+int mpdiv_debug_phases(unsigned long long out[64], int reset)
+{
+    if (cudaDeviceSynchronize() != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(out, g_phase, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (reset) {
+        unsigned long long z[64] = {0};
+        if (cudaMemcpyToSymbol(g_phase, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    }
+    return MPDIV_OK;
+}
+#endif
 
 int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream)
 {
