@@ -25,6 +25,22 @@
 #pragma once
 #include "mp_block.cuh"
 
+// Tuning builds (-DMPDIV_PHASE_TIMING) split the cycles of block 0 by sub-phase; see mp_div.cuh.
+#ifdef MPDIV_PHASE_TIMING
+__device__ unsigned long long g_sub[64];
+__device__ long long g_sub_t0;
+#define SUBPHASE(i)                                                     \
+    do {                                                                \
+        if (blockIdx.x == 0 && threadIdx.x == 0) {                      \
+            const long long t_ = clock64();                             \
+            g_sub[(i)] += (unsigned long long)(t_ - g_sub_t0);          \
+            g_sub_t0 = t_;                                              \
+        }                                                               \
+    } while (0)
+#else
+#define SUBPHASE(i) do { } while (0)
+#endif
+
 namespace mpd {
 
 // four limb products of one parity class of row a: the 8-limb window held in the four 64-bit
@@ -106,22 +122,69 @@ __device__ __forceinline__ void tile_mac(DiagAcc &s, const uint32_t (&a)[8], con
     tile_row<7>(s, a[7], b);
 }
 
+// d[0..N) += x[0..N) + cin as ONE add.cc/addc.cc chain (N = 8 or 9); returns the carry out.
+template <int N>
+__device__ __forceinline__ uint32_t acc_chain(uint32_t *d, const uint32_t *x, uint32_t cin)
+{
+    static_assert(N == 8 || N == 9, "chain length");
+    uint32_t c;
+    if (N == 8) {
+        asm("add.cc.u32 %8, %17, 0xffffffff;\n\t"
+            "addc.cc.u32 %0, %0, %9;\n\t"
+            "addc.cc.u32 %1, %1, %10;\n\t"
+            "addc.cc.u32 %2, %2, %11;\n\t"
+            "addc.cc.u32 %3, %3, %12;\n\t"
+            "addc.cc.u32 %4, %4, %13;\n\t"
+            "addc.cc.u32 %5, %5, %14;\n\t"
+            "addc.cc.u32 %6, %6, %15;\n\t"
+            "addc.cc.u32 %7, %7, %16;\n\t"
+            "addc.u32 %8, 0, 0;"
+            : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3]), "+r"(d[4]), "+r"(d[5]), "+r"(d[6]), "+r"(d[7]),
+              "=&r"(c)
+            : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]), "r"(cin));
+    } else {
+        asm("add.cc.u32 %9, %19, 0xffffffff;\n\t"
+            "addc.cc.u32 %0, %0, %10;\n\t"
+            "addc.cc.u32 %1, %1, %11;\n\t"
+            "addc.cc.u32 %2, %2, %12;\n\t"
+            "addc.cc.u32 %3, %3, %13;\n\t"
+            "addc.cc.u32 %4, %4, %14;\n\t"
+            "addc.cc.u32 %5, %5, %15;\n\t"
+            "addc.cc.u32 %6, %6, %16;\n\t"
+            "addc.cc.u32 %7, %7, %17;\n\t"
+            "addc.cc.u32 %8, %8, %18;\n\t"
+            "addc.u32 %9, 0, 0;"
+            : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3]), "+r"(d[4]), "+r"(d[5]), "+r"(d[6]), "+r"(d[7]),
+              "+r"(d[8]), "=&r"(c)
+            : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]), "r"(x[8]),
+              "r"(cin));
+    }
+    return c;
+}
+
+// d += x over 17 limbs (no carry out: the top limb of a diagonal sum is small)
+__device__ __forceinline__ void add17(uint32_t (&d)[17], const uint32_t (&x)[17])
+{
+    const uint32_t c = acc_chain<8>(d, x, 0u);
+    acc_chain<9>(d + 8, x + 8, c);
+}
+
 // D[0..16] = E + (O << 1 limb) + (CY << 8 limbs).
 __device__ __forceinline__ void diag_finish(const DiagAcc &s, uint32_t (&d)[17])
 {
-    uint32_t e[16], o[14];
+    uint32_t e[17], o[17];
 #pragma unroll
     for (int i = 0; i < 8; i++) { e[2 * i] = (uint32_t)s.E[i]; e[2 * i + 1] = (uint32_t)(s.E[i] >> 32); }
+    e[16] = 0u;
+    o[0] = 0u;
 #pragma unroll
-    for (int i = 0; i < 7; i++) { o[2 * i] = (uint32_t)s.O[i]; o[2 * i + 1] = (uint32_t)(s.O[i] >> 32); }
-    unsigned long long cy = 0;
-    d[0] = e[0];
+    for (int i = 0; i < 7; i++) { o[2 * i + 1] = (uint32_t)s.O[i]; o[2 * i + 2] = (uint32_t)(s.O[i] >> 32); }
+    o[15] = 0u; o[16] = 0u;
 #pragma unroll
-    for (int i = 1; i <= 16; i++) {
-        cy += (unsigned long long)(i < 16 ? e[i] : 0u) + (i - 1 < 14 ? o[i - 1] : 0u) + (i >= 8 ? s.CY[i - 8] : 0u);
-        d[i] = (uint32_t)cy;
-        cy >>= 32;
-    }
+    for (int i = 0; i < 17; i++) d[i] = e[i];
+    const uint32_t c = acc_chain<8>(d, o, 0u);                // limbs 0..7
+    acc_chain<9>(d + 8, o + 8, c);                            // limbs 8..16
+    acc_chain<9>(d + 8, s.CY, 0u);                            // chain-end carries enter at limb 8
 }
 
 // 8 limbs from shared memory at the 32-bit shared-window address `saddr` (16-byte aligned).
@@ -158,28 +221,24 @@ struct MulScratch {
 // T / 4 (cyclically: the up-ramp / plateau / down-ramp profile of a full product balances over the
 // passes; snake = true reverses odd passes, which balances the single ramp of a truncated product).
 // A pass that has fewer diagonals left than groups widens its groups (up to a whole warp).
-__device__ __forceinline__ void add17(uint32_t (&d)[17], const uint32_t (&x)[17])
-{
-    unsigned long long cy = 0;
-#pragma unroll
-    for (int i = 0; i < 17; i++) {
-        cy += (unsigned long long)d[i] + x[i];
-        d[i] = (uint32_t)cy;
-        cy >>= 32;
-    }
-}
-
 template <int T>
 __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
                                                   limb *P, limb *HI, uint32_t *OV, bool snake)
 {   // everything by value: a reference argument of a noinline function lives in local memory
-    constexpr int G0 = T / 4;                       // diagonals per full pass (4 lanes each)
+    // lanes per diagonal: 4 for long diagonals, fewer when a diagonal has only a tile or two (the shuffle
+    // reduction then costs more than it saves); a pass with spare threads widens its groups, but never
+    // beyond one lane per two tiles
+    const int maxlen = min(Na, Nb);
+    const int sh0 = maxlen <= 2 ? 0 : (maxlen <= 4 ? 1 : 2);
+    int shmax = sh0;
+    while (shmax < 5 && (2 << shmax) <= maxlen) ++shmax;
+    const int G0 = T >> sh0;                        // diagonals per full pass
     int pass = 0;
     uint32_t tiles = 0;
     for (int base = Klo; base < Kd; base += G0, ++pass) {
         const int ndiag = min(G0, Kd - base);
-        int sh = 2;
-        while (sh < 5 && (ndiag << (sh + 1)) <= T) ++sh;
+        int sh = sh0;
+        while (sh < shmax && (ndiag << (sh + 1)) <= T) ++sh;
         const int C = 1 << sh;
         const int g = (int)threadIdx.x >> sh, c = (int)threadIdx.x & (C - 1);
         const bool act = g < ndiag;
@@ -294,8 +353,11 @@ __device__ __forceinline__ void mul_full(const limb *A, int na, const limb *Bp, 
 {
     const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
     const int Kd = Na + Nb - 1;
+    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, false);
+    SUBPHASE(49);
     blk.parity = mul_resolve<T>(P, 0, Kd, Na + Nb, ms.HI, ms.OV, ms.C3, blk);
+    SUBPHASE(50);
 }
 
 template <int T>
@@ -306,8 +368,11 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
     const int Kfull = Na + Nb;
     const int Kc = min((L + TILE - 1) / TILE, Kfull);
     const int Kd = min(Kc, Kfull - 1);
+    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, Kd < Kfull - 1);
+    SUBPHASE(49);
     blk.parity = mul_resolve<T>(P, 0, Kd, Kc, ms.HI, ms.OV, ms.C3, blk);
+    SUBPHASE(50);
 }
 
 // Clipped ("range") product: only tile diagonals Klo <= K < Khi are computed, so the result is
@@ -326,8 +391,11 @@ __device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, 
     const int Kd = min(Kc, Kfull - 1);
     limb *Pd = P - TILE * Klo, *HId = ms.HI - TILE * Klo;
     uint32_t *OVd = ms.OV - Klo, *C3d = ms.C3 - Klo;
+    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, true);
+    SUBPHASE(49);
     blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
+    SUBPHASE(50);
     return TILE * max(Kc - Klo, 0);
 }
 

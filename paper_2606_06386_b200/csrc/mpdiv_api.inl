@@ -392,10 +392,14 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
 int mpdiv_debug_phases(unsigned long long out[64], int reset)
 {
     if (cudaDeviceSynchronize() != cudaSuccess) return MPDIV_ERR_CUDA;
+    unsigned long long sub[64];
     if (cudaMemcpyFromSymbol(out, g_phase, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(sub, g_sub, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    for (int i = 48; i < 64; i++) out[i] = sub[i];       // slots 48.. carry the multiplier sub-phases
     if (reset) {
         unsigned long long z[64] = {0};
         if (cudaMemcpyToSymbol(g_phase, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
+        if (cudaMemcpyToSymbol(g_sub, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
     }
     return MPDIV_OK;
 }
