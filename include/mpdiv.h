@@ -101,9 +101,13 @@ int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_lim
 
 /*
  * Host-buffer form of mpdiv_batch for end-to-end use: u, v, q, r are HOST pointers (pinned memory
- * recommended); `workspace` is a caller-owned DEVICE buffer of at least
- * mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch) bytes.  Enqueues H2D copies of u and v, the
- * division, and D2H copies of q and r on `stream`, then returns; the caller synchronises.
+ * recommended; pageable memory works but serialises the copies); `workspace` is a caller-owned DEVICE
+ * buffer of at least mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch) bytes.  The batch is cut into
+ * chunks of about one wave of the kernel; the H2D copy of chunk i+1 and the D2H copy of chunk i-1
+ * overlap the division of chunk i on two library-owned helper streams (created on first use, never
+ * destroyed).  Everything is ordered after the work already enqueued on `stream`, and `stream`
+ * completes only after the last D2H copy: the caller synchronises `stream` and reads q, r.
+ * Reuse of the same events makes concurrent calls from several host threads unsupported.
  */
 size_t mpdiv_host_workspace_bytes(int u_limbs, int v_limbs, int batch);
 int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host, int v_limbs,

@@ -179,7 +179,7 @@ int threads_for(int limbs)
         if (t == 64 || t == 128 || t == 256 || t == 512) return t;
     }
     if (limbs <= 128) return 64;
-    if (limbs <= 512) return 128;
+    if (limbs <= 2048) return 128;      // four blocks per SM overlap the latency-bound early iterations
     if (limbs <= 4096) return 256;
     return 512;
 }

@@ -284,6 +284,18 @@ int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, 
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
+// divisions one wave of the division kernel holds on the whole GPU (blocks per SM x SMs)
+template <int T>
+int div_wave(int u_limbs, int v_limbs, int clip)
+{
+    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    const size_t bytes = (size_t)L.total_words * 4;
+    if (set_smem(mpdiv_kernel<T>, bytes) != MPDIV_OK) return 0;
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mpdiv_kernel<T>, T, bytes) != cudaSuccess) return 0;
+    return nb * g_sm_count;
+}
+
 template <int T>
 int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st, int clip)
 {
@@ -373,18 +385,62 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     if (rc != MPDIV_OK) return rc;
     if (!workspace || !aligned16(workspace)) return MPDIV_ERR_BAD_ARG;
     if (workspace_bytes < mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch)) return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    const size_t ub = (size_t)batch * u_limbs * 4, vb = (size_t)batch * v_limbs * 4;
     uint32_t *du = static_cast<uint32_t *>(workspace);
     uint32_t *dv = du + (size_t)batch * u_limbs;
     uint32_t *dq = dv + (size_t)batch * v_limbs;
     uint32_t *dr = dq + (size_t)batch * u_limbs;
-    if (cudaMemcpyAsync(du, u_host, ub, cudaMemcpyHostToDevice, st) != cudaSuccess) return MPDIV_ERR_CUDA;
-    if (cudaMemcpyAsync(dv, v_host, vb, cudaMemcpyHostToDevice, st) != cudaSuccess) return MPDIV_ERR_CUDA;
-    rc = mpdiv_batch(du, u_limbs, dv, v_limbs, dq, dr, batch, stream);
-    if (rc != MPDIV_OK) return rc;
-    if (cudaMemcpyAsync(q_host, dq, ub, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MPDIV_ERR_CUDA;
-    if (cudaMemcpyAsync(r_host, dr, vb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MPDIV_ERR_CUDA;
+
+    // Chunks of about one wave of the kernel: the upload of chunk i+1 and the download of chunk i-1
+    // overlap the division of chunk i (two helper streams, created once; events order the three).
+    int wave = 0;
+    switch (threads_for(u_limbs)) {
+        case 64: wave = div_wave<64>(u_limbs, v_limbs, 1); break;
+        case 128: wave = div_wave<128>(u_limbs, v_limbs, 1); break;
+        case 256: wave = div_wave<256>(u_limbs, v_limbs, 1); break;
+        default: wave = div_wave<512>(u_limbs, v_limbs, 1); break;
+    }
+    if (wave <= 0) return MPDIV_ERR_UNSUPPORTED;
+    constexpr int MAXC = 8;
+    int chunk = wave;
+    if ((batch + chunk - 1) / chunk > MAXC) chunk = ((batch + MAXC - 1) / MAXC + wave - 1) / wave * wave;
+    const int nchunks = (batch + chunk - 1) / chunk;
+
+    static cudaStream_t s_in = nullptr, s_out = nullptr;
+    static cudaEvent_t ev_start = nullptr, ev_in[MAXC], ev_k[MAXC], ev_done = nullptr;
+    if (!s_in) {
+        if (cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
+        if (cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
+        if (cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
+        if (cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
+        for (int i = 0; i < MAXC; i++) {
+            if (cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
+            if (cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
+        }
+    }
+#define MPDIV_CK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return MPDIV_ERR_CUDA; } } while (0)
+    MPDIV_CK(cudaEventRecord(ev_start, st));                  // the helpers start after earlier work on `stream`
+    MPDIV_CK(cudaStreamWaitEvent(s_in, ev_start, 0));
+    MPDIV_CK(cudaStreamWaitEvent(s_out, ev_start, 0));
+    for (int c = 0; c < nchunks; c++) {
+        const size_t lo = (size_t)c * chunk;
+        const int cnt = (int)((size_t)batch - lo < (size_t)chunk ? (size_t)batch - lo : (size_t)chunk);
+        const size_t uo = lo * u_limbs, vo = lo * v_limbs;
+        MPDIV_CK(cudaMemcpyAsync(du + uo, u_host + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyHostToDevice, s_in));
+        MPDIV_CK(cudaMemcpyAsync(dv + vo, v_host + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyHostToDevice, s_in));
+        MPDIV_CK(cudaEventRecord(ev_in[c], s_in));
+        MPDIV_CK(cudaStreamWaitEvent(st, ev_in[c], 0));
+        rc = mpdiv_batch(du + uo, u_limbs, dv + vo, v_limbs, dq + uo, dr + vo, cnt, stream);
+        if (rc != MPDIV_OK) return rc;
+        MPDIV_CK(cudaEventRecord(ev_k[c], st));
+        MPDIV_CK(cudaStreamWaitEvent(s_out, ev_k[c], 0));
+        MPDIV_CK(cudaMemcpyAsync(q_host + uo, dq + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyDeviceToHost, s_out));
+        MPDIV_CK(cudaMemcpyAsync(r_host + vo, dr + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyDeviceToHost, s_out));
+    }
+    MPDIV_CK(cudaEventRecord(ev_done, s_out));
+    MPDIV_CK(cudaStreamWaitEvent(st, ev_done, 0));            // `stream` completes when the last download has
+#undef MPDIV_CK
     return MPDIV_OK;
 }
 
