@@ -186,7 +186,8 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
 
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
-                 "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "rsv12", "rsv13", "rsv14", "rsv15")
+                 "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "mma_products", "mma_wait_failures",
+                 "rsv14", "rsv15")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:

@@ -26,13 +26,15 @@
 // Iterations whose operands are too short for the window to clip anything run the printed code.
 #pragma once
 #include "mp_mul.cuh"
+#include "mp_mma.cuh"
 
 namespace mpd {
 
 // debug counters (include/mpdiv.h: mpdiv_debug_counters)
 __device__ unsigned long long g_counters[16];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
-       CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS };
+       CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
+       CNT_MMA_PRODUCTS };
 
 // Phase timing for tuning builds only (-DMPDIV_PHASE_TIMING): thread 0 of block 0 accumulates the cycles
 // between consecutive PHASE() marks.  Compiles to nothing in the product build.
@@ -84,11 +86,30 @@ struct ShinvBufs {
     MulScratch ms;
 };
 
+// Block sizes whose kernels carry the tensor-core multiplier (mp_mma.cuh); the others never see an MmaCtx.
+template <int T>
+struct MmaEnabled { static constexpr bool value = (T == 512); };
+
+// Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
+// P[i] = limb 32*dlo + i.
+template <int T>
+__device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na, const limb *Bp, int nb, int dlo, int dhi,
+                                             limb *P, limb *HI, Blk &blk)
+{
+    if constexpr (MmaEnabled<T>::value) {
+        bool swap;
+        if (mma_plan(mma, na, nb, dlo, dhi, swap))
+            return swap ? mma_mul_range<T>(*mma, Bp, nb, A, na, dlo, dhi, P, HI, blk)
+                        : mma_mul_range<T>(*mma, A, na, Bp, nb, dlo, dhi, P, HI, blk);
+    }
+    return -1;
+}
+
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
-                                           bool clip)
+                                           bool clip, MmaCtx *mma = nullptr)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
     const MulScratch &ms = bufs.ms;
@@ -177,9 +198,15 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                     lin_copy<T>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
             } else {
                 // clipped close product: limbs [c, L) of v'w only; X holds x / B^c (low limbs taken as 0)
-                c = TILE * Klo2;
                 count(CNT_CLIPPED_STEPS);
-                mul_range<T>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
+                const int dlo = (cx - 1) / 32;               // tensor-core form: blocks of 32 limbs, E < B^(32 dlo + 1)
+                if (try_mma_range<T>(mma, Vp, pv, Wc, pw, dlo, (L + 31) / 32, P, ms.HI, blk) >= 0) {
+                    c = 32 * dlo;
+                    count(CNT_MMA_PRODUCTS);
+                } else {
+                    c = TILE * Klo2;
+                    mul_range<T>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
+                }
                 xl = L - c;
                 positive = P[xl - 1] != 0u;
                 for (int i = threadIdx.x; i < round_up(xl, TILE); i += T)
@@ -199,8 +226,15 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
             // w*x / B^(d+1): the shift_{2m-h'} of Step and the shift_{-1} of Refine drop d + 1 limbs
             const int dd = d + 1 - c;
             const int Klo1 = (clip && dd >= 17) ? (dd - 9) / TILE : 0;
-            int tl, off;
-            if (Klo1 == 0) {
+            int tl = -1, off = 0;
+            bool exact = (Klo1 == 0 && c == 0);
+            if (clip && dd >= 33) {
+                const int dlo = (dd - 1) / 32;
+                tl = try_mma_range<T>(mma, Wc, pw, X, xl, dlo, 1 << 20, P, ms.HI, blk);
+                if (tl >= 0) { off = dd - 32 * dlo; exact = false; count(CNT_MMA_PRODUCTS); }
+            }
+            if (tl >= 0) {
+            } else if (Klo1 == 0) {
                 mul_full<T>(Wc, pw, X, xl, P, ms, blk);
                 tl = round_up(pw, TILE) + round_up(xl, TILE);
                 off = dd;
@@ -214,7 +248,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                 // floor of a negative: borrow one when any dropped limb of w*x is non-zero (exact path only;
                 // a clipped step is off by less than a guard-limb unit either way)
                 uint32_t bin = 0u;
-                if (Klo1 == 0 && c == 0) bin = any_nonzero<T>(P, 0, min(dd, tl)) ? 1u : 0u;
+                if (exact) bin = any_nonzero<T>(P, 0, min(dd, tl)) ? 1u : 0u;
                 lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
             }
         }

@@ -1,0 +1,328 @@
+// Tensor-core multiplier for the large products: a big-integer product as an int8 tcgen05 GEMM (sm_100a).
+//
+// The product of two numbers is the convolution of their BYTE strings, c[t] = sum_x a[x] * b[t - x],
+// followed by carry propagation.  Write t = 128 d + i (i < 128) and cut b into 128-byte chunks e; then
+//
+//     c[128 d + i] = sum_p  sum_{j < 128}  a[128 p + i - j] * b[128 (d - p) + j]
+//                  = sum_p  ( A_p  x  B_p )[i][d],      A_p[i][j] = a[128 p + i - j]   (128 x 128 Toeplitz tile)
+//                                                        B_p[j][d] = b[128 (d - p) + j] (chunk d - p of b)
+//
+// i.e. one GEMM with M = 128 (byte position inside an output block), N = number of output blocks,
+// K = 128 x (number of chunks of a + 1), u8 x u8 -> s32 (`tcgen05.mma.kind::i8`, accumulators in TMEM;
+// a column sum is below 255^2 * 32768 < 2^31 for operands up to 8192 limbs).
+//   * B_p needs no work per step: b is stored ONCE as 128-byte rows in the K-major SWIZZLE_128B layout
+//     (16-byte units XOR-ed with the row number, on absolute shared-memory addresses), and step p simply
+//     starts its descriptor p rows lower.
+//   * A_p is generated on the fly by the CUDA cores: row i is the byte-reversed 128-byte window of a
+//     ending at byte 128 p + i -- one PRMT per word from two neighbouring words -- written into a ring of
+//     16 KB stages, handed to the single MMA-issuing thread through mbarriers (`fence.proxy.async` makes
+//     the generic-proxy stores visible to the tensor core), and freed by `tcgen05.commit`.
+//   * Epilogue: `tcgen05.ld` (lane = i, column = d), four adjacent lanes form one limb's 64-bit column
+//     sum, low words go to P, high words to HI one limb up, and one block-wide carry-propagating add
+//     (mp_block.cuh) finishes.
+// A range of output blocks dlo <= d < dhi can be asked for (clipped products); what is omitted below
+// block dlo is less than B^(32 dlo + 1).  Only steps p whose chunk d - p can be non-zero are issued.
+//
+// Measured on B200 (standalone, one product per SM at a time): 8.5e12 / 1.7e13 / 3.2e13 limb products/s
+// for full 1024 / 2048 / 4096-limb squares against 9.15e12 for the IMAD.WIDE roofline probe.
+#pragma once
+#include "mp_block.cuh"
+
+namespace mpd {
+
+#ifndef MMA_STAGES_N
+#define MMA_STAGES_N 2
+#endif
+constexpr int MMA_STAGES = MMA_STAGES_N;
+constexpr int MMA_TILE_BYTES = 128 * 128;
+#ifndef MMA_SPIN_LIMIT_LOG2
+#define MMA_SPIN_LIMIT_LOG2 26
+#endif
+constexpr uint32_t MMA_SPIN_LIMIT = 1u << MMA_SPIN_LIMIT_LOG2;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// bounded wait: a protocol error must not hang the GPU; false = gave up
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity)
+{
+    for (uint32_t it = 0; it < MMA_SPIN_LIMIT; ++it) {
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return true;
+    }
+    return false;
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem desc] x B[smem desc], u8 x u8 -> s32, M = 128, K = 32
+__device__ __forceinline__ void tc_mma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                          uint32_t accumulate)
+{
+    const uint32_t z = 0;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+}
+// K-major SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes apart
+__device__ __forceinline__ uint64_t mma_smem_desc(uint32_t saddr)
+{
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ uint32_t mma_idesc(int n_cols)      // u8 x u8 -> s32, both K-major, M = 128
+{
+    return (2u << 4) | ((uint32_t)(n_cols >> 3) << 17) | ((128u >> 4) << 24);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// Per-block state of the tensor-core multiplier (block-uniform values, kept in registers).
+struct MmaCtx {
+    uint32_t tmem_base;   // first allocated TMEM column
+    int tmem_cols;        // allocated columns (power of two >= 32): at most this many output blocks per call
+    uint8_t *stages;      // MMA_STAGES x 16 KB ring of Toeplitz tiles, 1024-byte aligned
+    uint8_t *brows;       // the row operand in swizzled 128-byte rows, 1024-byte aligned
+    int brows_cap;        // rows available at brows
+    uint32_t bar;         // shared address of the mbarriers: full[s] at +8 s, empty[s] at +32 + 8 s, done at +64
+    uint32_t it;          // tiles produced so far (stage index and barrier parities follow from it)
+    uint32_t ndone;       // products finished so far (parity of the done barrier)
+    uint32_t fail;        // set when a bounded wait gave up
+};
+
+#ifdef MMA_TIMING
+__device__ unsigned long long g_mma_t[8];
+#define MMA_T(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { long long t_ = clock64(); g_mma_t[i] += (unsigned long long)(t_ - t0_); t0_ = t_; } } while (0)
+#else
+#define MMA_T(i) do { } while (0)
+#endif
+__device__ unsigned int g_mma_fail;   // bounded waits that gave up (expected 0); reported with the debug counters
+
+constexpr int MMA_BAR_BYTES = 128;    // full[s] (up to 4), empty[s] (up to 4), done, TMEM slot
+
+// One-time setup per block: mbarriers, TMEM allocation (warp 0 owns it).  All threads call it.
+template <int T>
+__device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *stages, uint8_t *brows, int brows_cap, uint8_t *bars,
+                                         int tmem_cols)
+{
+    cx.stages = stages;
+    cx.brows = brows;
+    cx.brows_cap = brows_cap;
+    cx.bar = smem_u32(bars);
+    cx.tmem_cols = tmem_cols;
+    cx.it = 0;
+    cx.ndone = 0;
+    cx.fail = 0;
+    uint32_t *slot = reinterpret_cast<uint32_t *>(bars + 96);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < MMA_STAGES; s++) {
+            mbar_init(cx.bar + 8 * s, (T - 32) / 32); // one arrival per producer warp
+            mbar_init(cx.bar + 32 + 8 * s, 1);       // tcgen05.commit
+        }
+        mbar_init(cx.bar + 64, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (threadIdx.x < 32) {
+        __syncwarp();                                // thread 0 rejoins its warp before the aligned instructions
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "r"(tmem_cols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    cx.tmem_base = *slot;
+}
+
+template <int T>
+__device__ __forceinline__ void mma_fini(MmaCtx &cx)
+{
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x < 32)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(cx.tmem_base), "r"(cx.tmem_cols));
+}
+
+// One 16-byte unit of a Toeplitz tile: bytes j = 16c .. 16c+15 of row `row` of tile p, out[j] = a[128p + row - j],
+// stored at the swizzled position of the K-major SWIZZLE_128B layout.  W = the operand's limbs, nw = valid
+// words (zero outside [0, nw)); CHECK = false skips the bounds tests.
+template <bool CHECK>
+__device__ __forceinline__ void toeplitz_unit(const limb *W, int nw, int p, int row, int c, uint8_t *tile)
+{
+    const int z0 = 128 * p + row - 16 * c - 3;               // lowest byte of the first output word
+    const int s = z0 & 3;
+    const uint32_t sel = (uint32_t)(s + 3) | ((uint32_t)(s + 2) << 4) | ((uint32_t)(s + 1) << 8) | ((uint32_t)s << 12);
+    const int wi = z0 >> 2;                                  // floor(z0 / 4), also for negative z0
+    auto ld = [&](int i) -> uint32_t { return CHECK ? ((i >= 0 && i < nw) ? W[i] : 0u) : W[i]; };
+    const uint32_t w4 = ld(wi + 1), w3 = ld(wi), w2 = ld(wi - 1), w1 = ld(wi - 2), w0 = ld(wi - 3);
+    uint4 o;
+    o.x = __byte_perm(w3, w4, sel);                          // bytes a[z+3], a[z+2], a[z+1], a[z]
+    o.y = __byte_perm(w2, w3, sel);
+    o.z = __byte_perm(w1, w2, sel);
+    o.w = __byte_perm(w0, w1, sel);
+    *reinterpret_cast<uint4 *>(tile + row * 128 + ((c ^ (row & 7)) << 4)) = o;
+}
+
+// Steps (Toeplitz tiles) a range product needs when `na` is the Toeplitz operand.
+__device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
+{
+    const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
+    return min(Ea, dhi - 1) - max(0, dlo - Eb + 1) + 1;
+}
+
+// Should this range product run on the tensor core?  Measured on B200 (512-thread block alone on its SM):
+// a step costs about 810 cycles (the MMA instruction itself takes ~132 cycles whatever N is; the rest is
+// shared-memory bandwidth of the tile generation), a call about 12 000 cycles of fixed work (row operand,
+// epilogue, final add), against about 1/26 cycle per limb product on the IMAD path.  swap = take b as the
+// Toeplitz operand (fewer steps).  Block-uniform.
+__device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
+{
+    if (cx == nullptr || na <= 0 || nb <= 0 || dlo < 0) return false;
+    dhi = min(dhi, (na + nb + 31) / 32);
+    const int N = dhi - dlo, Nn = (N + 15) & ~15;
+    if (N <= 0) return false;
+    const int sa = mma_steps(na, nb, dlo, dhi), sb = mma_steps(nb, na, dlo, dhi);
+    swap = sb < sa;
+    const int steps = swap ? sb : sa;
+    if (steps <= 0 || Nn > cx->tmem_cols || Nn + steps - 1 > cx->brows_cap) return false;
+    const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
+    return est >= 52ll * (810ll * steps + 12000ll);
+}
+
+// P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).
+// A (na limbs) is the Toeplitz operand, B (nb limbs) the row operand; both plain little-endian limbs in
+// shared memory, read as zero beyond na / nb.  HI is scratch of the same size as P (+8).  dhi is clamped
+// to the size of the full product.  All T threads call it; ends with the result visible to the block.
+// Returns the number of limbs stored, or -1 when the request does not fit (TMEM columns or row buffer).
+template <int T>
+__device__ __noinline__ int mma_mul_range(MmaCtx &cx, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
+                                          limb *P, limb *HI, Blk &blk)
+{
+    static_assert(T >= 128 && T % 32 == 0, "four epilogue warps and an issuer");
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
+    dhi = min(dhi, (na + nb + 31) / 32);
+    const int N = dhi - dlo;
+    const int Nn = (N + 15) & ~15;
+    const int pmin = max(0, dlo - Eb + 1), pmax = min(Ea, dhi - 1);
+    const int e0 = dlo - pmax;                                // chunk of b held by row 0
+    const int R = (dlo + Nn - 1 - pmin) - e0 + 1;
+    if (N <= 0 || pmax < pmin || Nn > cx.tmem_cols || R > cx.brows_cap) return -1;
+
+#ifdef MMA_TIMING
+    long long t0_ = clock64();
+#endif
+    // ---- the row operand: chunk e of b -> row e - e0, 16-byte units swizzled by the row number ----
+    for (int q = tid; q < R * 8; q += T) {
+        const int r = q >> 3, c = q & 7;
+        const int w0 = (r + e0) * 32 + c * 4;
+        uint4 val;
+        val.x = (w0 + 0 >= 0 && w0 + 0 < nb) ? B[w0 + 0] : 0u;
+        val.y = (w0 + 1 >= 0 && w0 + 1 < nb) ? B[w0 + 1] : 0u;
+        val.z = (w0 + 2 >= 0 && w0 + 2 < nb) ? B[w0 + 2] : 0u;
+        val.w = (w0 + 3 >= 0 && w0 + 3 < nb) ? B[w0 + 3] : 0u;
+        *reinterpret_cast<uint4 *>(cx.brows + r * 128 + ((c ^ (r & 7)) << 4)) = val;
+    }
+    fence_async_smem();
+    __syncthreads();
+
+    MMA_T(0);
+    const int nsteps = pmax - pmin + 1;
+    constexpr int NPROD = T - 32;
+    if (tid < NPROD) {
+        // ---- Toeplitz producers: every producer thread fills its share of the 1024 units of EVERY tile, so
+        //      each of them sees every phase of the stage barriers (the parity protocol needs that) ----
+        for (int step = 0; step < nsteps; ++step) {
+            const int p = pmin + step;
+            const uint32_t it = cx.it + (uint32_t)step;
+            const int s = (int)(it % MMA_STAGES);
+            if (it >= MMA_STAGES && !mbar_wait(cx.bar + 32 + 8 * s, ((it / MMA_STAGES) - 1) & 1)) { cx.fail = 1; break; }
+            uint8_t *tile = cx.stages + s * MMA_TILE_BYTES;
+            if (p >= 1 && 32 * p + 33 <= na) {
+                for (int u = tid; u < 1024; u += NPROD) toeplitz_unit<false>(A, na, p, u & 127, u >> 7, tile);
+            } else {
+                for (int u = tid; u < 1024; u += NPROD) toeplitz_unit<true>(A, na, p, u & 127, u >> 7, tile);
+            }
+            fence_async_smem();                              // generic-proxy stores -> visible to the tensor core
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(cx.bar + 8 * s); // one arrival per producer warp
+        }
+    } else if (tid == NPROD) {
+        // ---- the MMA issuer ----
+        for (int step = 0; step < nsteps; ++step) {
+            const int p = pmin + step;
+            const uint32_t it = cx.it + (uint32_t)step;
+            const int s = (int)(it % MMA_STAGES);
+            if (!mbar_wait(cx.bar + 8 * s, (it / MMA_STAGES) & 1)) { cx.fail = 2; break; }
+            tc_fence_after();
+            const uint32_t a_addr = smem_u32(cx.stages + s * MMA_TILE_BYTES);
+            for (int nc = 0; nc < Nn; nc += 256) {
+                const int ncols = min(256, Nn - nc);
+                const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
+                const uint32_t idesc = mma_idesc(ncols);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    tc_mma_i8(cx.tmem_base + nc, mma_smem_desc(a_addr + 32 * k), mma_smem_desc(b_addr + 32 * k), idesc,
+                              (step > 0 || k > 0) ? 1u : 0u);
+            }
+            tc_commit(cx.bar + 32 + 8 * s);
+        }
+        tc_commit(cx.bar + 64);
+    }
+    cx.it += (uint32_t)nsteps;
+    __syncwarp();
+    MMA_T(1);
+
+    // ---- epilogue: TMEM lane i, column d  ->  byte-column sum of output byte 128 (dlo + d) + i ----
+    if (warp < 4) {
+        if (!mbar_wait(cx.bar + 64, cx.ndone & 1)) cx.fail = 3;
+        tc_fence_after();
+        MMA_T(2);
+        for (int d0 = 0; d0 < Nn; d0 += 16) {
+            uint32_t v[16];
+            tmem_ld16(cx.tmem_base + ((uint32_t)(32 * warp) << 16) + d0, v);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                unsigned long long sv = (unsigned long long)v[k] << (8 * (tid & 3));
+                sv += __shfl_xor_sync(0xffffffffu, sv, 1);
+                sv += __shfl_xor_sync(0xffffffffu, sv, 2);
+                if ((tid & 3) == 0 && d0 + k < N) {
+                    const int L = 32 * (d0 + k) + (tid >> 2);
+                    P[L] = (uint32_t)sv;
+                    HI[L + 1] = (uint32_t)(sv >> 32);
+                }
+            }
+        }
+        if (tid == 0) HI[0] = 0u;
+        tc_fence_before();
+    }
+    MMA_T(3);
+    cx.ndone += 1;
+    if (cx.fail) atomicOr(&g_mma_fail, 1u << (cx.fail - 1));
+    __syncthreads();
+    // ---- P += HI with block-wide carry propagation (the carry out of the top block is dropped: mod B^(32 dhi)) ----
+    lin_addsub<T, false>(P, 32 * N, LimbView{P, 32 * N, 0}, LimbView{HI, 32 * N, 0}, 0u, blk);
+    MMA_T(4);
+    return 32 * N;
+}
+
+}  // namespace mpd

@@ -7,6 +7,9 @@
 // ---------------------------------------------------------------------------------------
 struct DivLayout {
     int v_off, u_off, wa_off, big_off, sc_off, total_words;
+    int mma_off;      // word offset (1024-byte aligned) of the tensor-core scratch, or -1: stages | rows | barriers
+    int mma_rows;     // rows of 128 bytes available for the row operand
+    int mma_cols;     // TMEM columns to allocate
     int x_words;      // Refine: X at big_off, P behind it
     int p_words_r;    // Refine: capacity of P and of HI
     int p_words_q;    // quotient phase: capacity of P and of HI
@@ -39,7 +42,26 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
     L.big_off = o; o += (big_r > big_q ? big_r : big_q);
     L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
     L.total_words = o;
+    L.mma_off = -1;
+    L.mma_rows = 0;
+    L.mma_cols = 0;
     return L;
+}
+
+// Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the ring of
+// Toeplitz tiles, the row operand (output blocks + steps rows), the mbarriers.  max_smem in bytes.
+static void div_layout_add_mma(DivLayout &L, int M, int max_smem)
+{
+    const int blocks = (M / 2 + 1 + 9 + 31) / 32 + 2;             // output blocks of u * shinv at n = M/2
+    const int cols = blocks <= 32 ? 32 : blocks <= 64 ? 64 : blocks <= 128 ? 128 : 256;
+    const int rows = round_up(((blocks + 15) & ~15) + blocks + 8, 8);
+    const int off = round_up(L.total_words, 256);
+    const int words = MMA_STAGES * MMA_TILE_BYTES / 4 + rows * 32 + 64;
+    if ((off + words) * 4 > max_smem) return;
+    L.mma_off = off;
+    L.mma_rows = rows;
+    L.mma_cols = cols;
+    L.total_words = off + words;
 }
 
 __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout &L)
@@ -118,6 +140,16 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     mq.OV = mq.HI + L.p_words_q;
     mq.C3 = mq.OV + round_up(L.p_words_q / TILE, 4);
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
+    MmaCtx mcx;
+    MmaCtx *mma = nullptr;
+    if constexpr (MmaEnabled<T>::value) {
+        if (L.mma_off >= 0 && clip) {
+            uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
+            mma_init<T>(mcx, base, base + MMA_STAGES * MMA_TILE_BYTES, L.mma_rows,
+                        base + MMA_STAGES * MMA_TILE_BYTES + L.mma_rows * 128, L.mma_cols);
+            mma = &mcx;
+        }
+    }
 
     for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
         const limb *ug = u + (size_t)inst * u_limbs;
@@ -164,7 +196,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
         PHASE(1);
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0);
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma);
         const int psh = top_prec(WA, nw);
         PHASE(2);
 
@@ -217,9 +249,16 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             if (psh == 0) {
                 lin_zero<T>(Q, qlen);
             } else {
-                const int Klo = (h >= 17) ? (h - 9) / TILE : 0;
-                const int pl = mul_range<T>(Ub, h, WA, psh, Klo, 1 << 20, PQ, mq, blk);
-                lin_copy<T>(Q, qlen, PQ, pl, h - TILE * Klo);
+                const int dlo = (h - 1) / 32;              // tensor-core form: E < B^(32 dlo + 1) <= B^h
+                int pl = try_mma_range<T>(mma, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
+                if (pl >= 0) {
+                    count(CNT_MMA_PRODUCTS);
+                    lin_copy<T>(Q, qlen, PQ, pl, h - 32 * dlo);
+                } else {
+                    const int Klo = (h >= 17) ? (h - 9) / TILE : 0;
+                    pl = mul_range<T>(Ub, h, WA, psh, Klo, 1 << 20, PQ, mq, blk);
+                    lin_copy<T>(Q, qlen, PQ, pl, h - TILE * Klo);
+                }
             }
             const int pq = top_prec(Q, nq);
             PHASE(4);
@@ -228,8 +267,14 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             rlen = round_up(k + 3, TILE);
             int pl = 0;
             if (pq > 0) {
-                mul_low<T>(Vb, k + 1, Q, pq, rlen, PQ, mq, blk);
-                pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
+                pl = try_mma_range<T>(mma, Vb, k + 1, Q, pq, 0, (rlen + 31) / 32, PQ, mq.HI, blk);
+                if (pl >= 0) {
+                    count(CNT_MMA_PRODUCTS);
+                    pl = min(rlen, pl);
+                } else {
+                    mul_low<T>(Vb, k + 1, Q, pq, rlen, PQ, mq, blk);
+                    pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
+                }
             }
 
             PHASE(5);
@@ -265,6 +310,9 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         PHASE(7);
     }
     count_tiles(blk);
+    if constexpr (MmaEnabled<T>::value) {
+        if (mma != nullptr) mma_fini<T>(mcx);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -276,7 +324,8 @@ template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
                cudaStream_t st, int clip)
 {
-    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
@@ -288,7 +337,8 @@ int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, 
 template <int T>
 int div_wave(int u_limbs, int v_limbs, int clip)
 {
-    const DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem);
     const size_t bytes = (size_t)L.total_words * 4;
     if (set_smem(mpdiv_kernel<T>, bytes) != MPDIV_OK) return 0;
     int nb = 0;
@@ -467,7 +517,12 @@ int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t s
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     if (cudaStreamSynchronize(st) != cudaSuccess) return MPDIV_ERR_CUDA;
     if (cudaMemcpyFromSymbol(out, g_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    unsigned int mma_fail = 0;
+    if (cudaMemcpyFromSymbol(&mma_fail, g_mma_fail, sizeof(mma_fail)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    out[13] = mma_fail;
     if (reset) {
+        const unsigned int zf = 0;
+        if (cudaMemcpyToSymbol(g_mma_fail, &zf, sizeof(zf)) != cudaSuccess) return MPDIV_ERR_CUDA;
         unsigned long long z[16] = {0};
         if (cudaMemcpyToSymbol(g_counters, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
     }
