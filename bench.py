@@ -220,6 +220,18 @@ def per_config_table(binding, flush, peak_products: float):
         b2 = b1[:, :nn].contiguous()
         c2 = torch.empty((b, 2 * nn), dtype=torch.int32, device="cuda")
         t_m2 = float(np.median(time_steps(lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2), 25, 3, flush)))
+        # the same two products on the tensor-core engine (int8 tcgen05), where it fits
+        t_m1_tc = t_m2_tc = None
+        try:
+            t_m1_tc = float(np.median(time_steps(
+                lambda: binding.mpmul_batch(a1, b1, m, c1, engine=binding.ENGINE_TENSOR), 25, 3, flush)))
+        except binding.MpdivError:
+            pass
+        try:
+            t_m2_tc = float(np.median(time_steps(
+                lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2, engine=binding.ENGINE_TENSOR), 25, 3, flush)))
+        except binding.MpdivError:
+            pass
         wl = (m + 1 + 3) // 4 * 4
         w = torch.empty((b, wl), dtype=torch.int32, device="cuda")
         t_sh = float(np.median(time_steps(lambda: binding.shinv_batch(dv, m, wl, w), 25, 3, flush)))
@@ -232,6 +244,9 @@ def per_config_table(binding, flush, peak_products: float):
             "mul_MxM_lowM_products_per_s": b * (m * (m + 1) / 2) / (t_m1 * 1e-3),
             "mul_nxn_full_products_per_s": b * nn * nn / (t_m2 * 1e-3),
             "hbm_GBps_div_io": b * 4 * (2 * m + 2 * n) / (t_div * 1e-3) / 1e9,
+            "mul_MxM_lowM_tensor_ms": t_m1_tc, "mul_nxn_full_tensor_ms": t_m2_tc,
+            "mul_nxn_full_tensor_products_per_s": (b * nn * nn / (t_m2_tc * 1e-3)) if t_m2_tc else None,
+            "tensor_over_imad_speedup_nxn_full": (t_m2 / t_m2_tc) if t_m2_tc else None,
             "printed_variant_div_ms": t_div_printed, "printed_variant_div_per_s": b / (t_div_printed * 1e-3),
             "printed_variant_R1": t_div_printed / t_m1,
             "executed_limb_products_per_division": executed / b,
@@ -339,6 +354,9 @@ def run_ours(args):
                     "high part of v*q (PAPER.md:507, :542), so frac may exceed 1; pipe_frac counts what really ran",
             "executed_limb_products_per_launch": executed,
             "pipe_frac": executed / (kernel_ms * 1e-3) / peak_products,
+            "tensor_engine": "range products with enough work (u*shinv, v*q and the last doubling Refine step at "
+                             "2^18 bits) run as int8 tcgen05 GEMMs (csrc/mp_mma.cuh); per_config times both engines "
+                             "on the same products",
             "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
                                 "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
             "bound": "alu", "kernel": "mpdiv_kernel",

@@ -86,6 +86,21 @@ int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs,
                 uint32_t *c, int c_limbs, int batch, mpdiv_stream_t stream);
 
 /*
+ * Same product with an explicit engine.
+ *   MPMUL_ENGINE_IMAD    the block-level schoolbook multiplier on IMAD.WIDE (what mpmul_batch runs; the unit
+ *                        of the paper's cost model).
+ *   MPMUL_ENGINE_TENSOR  the product as an int8 tcgen05 GEMM: byte convolution with Toeplitz tiles generated
+ *                        on the fly, accumulators in TMEM (csrc/mp_mma.cuh).  The north star allows tensor
+ *                        cores only where measured faster: bench.py times both engines; mpdiv_batch uses this
+ *                        engine for its large range products at 2^18 bits.  MPDIV_ERR_UNSUPPORTED when the
+ *                        request needs more than 512 output blocks of 32 limbs or does not fit shared memory.
+ */
+#define MPMUL_ENGINE_IMAD 0
+#define MPMUL_ENGINE_TENSOR 1
+int mpmul_batch_ex(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs,
+                   uint32_t *c, int c_limbs, int batch, int engine, mpdiv_stream_t stream);
+
+/*
  * Whole shifted inverse as the division uses it, Alg. 1-2 and Theorem 2
  * (PAPER.md:160):   w_i = floor(B^h / v_i) + lambda_i,  lambda_i in {0, 1}
  * (lambda in {-1, 0, 1} for the clipped variant)

@@ -20,6 +20,7 @@ _VOIDP = ctypes.c_void_p
 OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
 VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
 VARIANT_DEFAULT = VARIANT_CLIPPED
+ENGINE_IMAD, ENGINE_TENSOR = 0, 1
 MAX_LIMBS = 8192
 
 
@@ -42,6 +43,7 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
         L.mpdiv_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, i, _VOIDP]
         L.shinv_batch_ex.argtypes = [_VOIDP, i, i, _VOIDP, i, i, i, _VOIDP]
+        L.mpmul_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, i, _VOIDP]
         L.mpmul_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, _VOIDP]
         L.shinv_batch.argtypes = [_VOIDP, i, i, _VOIDP, i, i, _VOIDP]
         L.mpdiv_host_workspace_bytes.argtypes = [i, i, i]
@@ -53,14 +55,14 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_version.restype = ctypes.c_char_p
         L.mpdiv_strerror.argtypes = [i]
         L.mpdiv_strerror.restype = ctypes.c_char_p
-        for name in ("mpdiv_batch", "mpdiv_batch_ex", "shinv_batch_ex", "mpmul_batch", "shinv_batch", "mpdiv_batch_host",
+        for name in ("mpdiv_batch", "mpdiv_batch_ex", "shinv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "mpdiv_batch_host",
                      "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_debug_counters"):
             getattr(L, name).restype = i
         _LIB = L
     return _LIB
 
 
-EXPORTS = ("mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
+EXPORTS = ("mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
            "mpdiv_debug_counters", "mpdiv_version", "mpdiv_strerror")
 
@@ -119,8 +121,9 @@ def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
     return q, r
 
 
-def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor | None = None, stream=None):
-    """c = (a * b) mod B^c_limbs per row."""
+def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor | None = None, stream=None,
+                engine: int | None = None):
+    """c = (a * b) mod B^c_limbs per row.  engine: None -> mpmul_batch (IMAD), else mpmul_batch_ex."""
     _check_dev(a, "a")
     _check_dev(b, "b")
     batch = a.shape[0]
@@ -129,8 +132,12 @@ def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor 
     if c is None:
         c = torch.empty((batch, c_limbs), dtype=a.dtype, device=a.device)
     _check_dev(c, "c")
-    _raise(lib().mpmul_batch(a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], c.data_ptr(), c_limbs, batch,
-                             _stream_ptr(stream)), "mpmul_batch")
+    if engine is None:
+        _raise(lib().mpmul_batch(a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], c.data_ptr(), c_limbs, batch,
+                                 _stream_ptr(stream)), "mpmul_batch")
+    else:
+        _raise(lib().mpmul_batch_ex(a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], c.data_ptr(), c_limbs, batch,
+                                    int(engine), _stream_ptr(stream)), "mpmul_batch_ex")
     return c
 
 

@@ -47,6 +47,7 @@ __device__ __forceinline__ void store_number(limb *__restrict__ dst, const limb 
 // ---------------------------------------------------------------------------------------
 struct MulLayout {
     int a_off, b_off, p_off, hi_off, ov_off, c3_off, sc_off, total_words;
+    int mma_off, mma_rows, mma_cols;     // tensor-core scratch (mp_mma.cuh), mma_off = -1 when absent
 };
 
 static MulLayout mul_layout(int a_limbs, int b_limbs, int c_limbs)
@@ -65,7 +66,43 @@ static MulLayout mul_layout(int a_limbs, int b_limbs, int c_limbs)
     L.c3_off = o; o += round_up(pc / TILE, 4);
     L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
     L.total_words = o;
+    L.mma_off = -1;
+    L.mma_rows = 0;
+    L.mma_cols = 0;
     return L;
+}
+
+// Scratch of the tensor-core engine for a product of a_limbs x b_limbs truncated to c_limbs; false if the
+// request does not fit (TMEM has 512 columns = 512 output blocks of 32 limbs; shared memory max_smem bytes).
+static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_limbs, int max_smem)
+{
+    const int full = (a_limbs + b_limbs + 31) / 32, want = (c_limbs + 31) / 32;
+    const int blocks = want < full ? want : full;
+    const int nn = (blocks + 15) & ~15;
+    if (nn > 512) return false;
+    const int cols = nn <= 32 ? 32 : nn <= 64 ? 64 : nn <= 128 ? 128 : nn <= 256 ? 256 : 512;
+    const int small = a_limbs < b_limbs ? a_limbs : b_limbs;
+    const int rows = round_up(nn + (small + 31) / 32 + 8, 8);
+    // P and HI must hold 32 limbs per output block
+    const int pc = 32 * blocks + 2 * TILE;
+    const int grow = pc - (L.hi_off - L.p_off);
+    if (grow > 0) {                       // re-lay P, HI, OV, C3, scratch with the larger product buffers
+        int o = L.p_off;
+        L.p_off = o; o += pc;
+        L.hi_off = o; o += pc;
+        L.ov_off = o; o += round_up(pc / TILE, 4);
+        L.c3_off = o; o += round_up(pc / TILE, 4);
+        L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
+        L.total_words = o;
+    }
+    const int off = round_up(L.total_words, 256);
+    const int words = MMA_STAGES * MMA_TILE_BYTES / 4 + rows * 32 + 64;
+    if ((off + words) * 4 > max_smem) return false;
+    L.mma_off = off;
+    L.mma_rows = rows;
+    L.mma_cols = cols;
+    L.total_words = off + words;
+    return true;
 }
 
 template <int T>
@@ -73,10 +110,20 @@ __global__ void __launch_bounds__(T, 512 / T)
 mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b, int b_limbs,
              limb *__restrict__ c, int c_limbs, int batch, MulLayout L)
 {
-    extern __shared__ __align__(16) uint32_t smem[];
+    extern __shared__ __align__(1024) uint32_t smem[];
     limb *A = smem + L.a_off, *Bs = smem + L.b_off, *P = smem + L.p_off;
     MulScratch ms{smem + L.hi_off, smem + L.ov_off, smem + L.c3_off};
     Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
+    MmaCtx mcx;
+    bool tensor = false;
+    if constexpr (MmaEnabled<T>::value) {
+        if (L.mma_off >= 0) {
+            uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
+            mma_init<T>(mcx, base, base + MMA_STAGES * MMA_TILE_BYTES, L.mma_rows,
+                        base + MMA_STAGES * MMA_TILE_BYTES + L.mma_rows * 128, L.mma_cols);
+            tensor = true;
+        }
+    }
 
     for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
         load_number<T>(A, a + (size_t)inst * a_limbs, a_limbs, round_up(a_limbs, TILE) + TILE);
@@ -85,7 +132,18 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
         const int na = prec_of<T>(A, a_limbs, blk);
         const int nb = prec_of<T>(Bs, b_limbs, blk);
         int valid = 0;
-        if (na > 0 && nb > 0) {
+        if constexpr (MmaEnabled<T>::value) {
+            if (tensor && na > 0 && nb > 0) {
+                // the operand with fewer 128-byte chunks becomes the Toeplitz operand (fewer MMA steps)
+                const int dhi = (c_limbs + 31) / 32;
+                const bool swap = mma_steps(nb, na, 0, dhi) < mma_steps(na, nb, 0, dhi);
+                valid = swap ? mma_mul_range<T>(mcx, Bs, nb, A, na, 0, dhi, P, ms.HI, blk)
+                             : mma_mul_range<T>(mcx, A, na, Bs, nb, 0, dhi, P, ms.HI, blk);
+                if (valid > c_limbs) valid = c_limbs;
+            }
+        }
+        if (valid > 0) {
+        } else if (na > 0 && nb > 0) {
             if (c_limbs >= na + nb) {
                 mul_full<T>(A, na, Bs, nb, P, ms, blk);
                 valid = round_up(na, TILE) + round_up(nb, TILE);
@@ -96,6 +154,9 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
         }
         store_number<T>(c + (size_t)inst * c_limbs, P, c_limbs, valid);
         __syncthreads();
+    }
+    if constexpr (MmaEnabled<T>::value) {
+        if (tensor) mma_fini<T>(mcx);
     }
 }
 
@@ -197,9 +258,11 @@ int set_smem(K kernel, size_t bytes)
 
 template <int T>
 int launch_mul(const limb *a, int a_limbs, const limb *b, int b_limbs, limb *c, int c_limbs, int batch,
-               cudaStream_t st)
+               cudaStream_t st, bool tensor = false)
 {
-    const MulLayout L = mul_layout(a_limbs, b_limbs, c_limbs);
+    MulLayout L = mul_layout(a_limbs, b_limbs, c_limbs);
+    if (tensor && !(MmaEnabled<T>::value && mul_layout_add_mma(L, a_limbs, b_limbs, c_limbs, g_max_smem)))
+        return MPDIV_ERR_UNSUPPORTED;
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpmul_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
@@ -214,6 +277,13 @@ extern "C" {
 int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, uint32_t *c, int c_limbs,
                 int batch, mpdiv_stream_t stream)
 {
+    return mpmul_batch_ex(a, a_limbs, b, b_limbs, c, c_limbs, batch, MPMUL_ENGINE_IMAD, stream);
+}
+
+int mpmul_batch_ex(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, uint32_t *c, int c_limbs,
+                   int batch, int engine, mpdiv_stream_t stream)
+{
+    if (engine != MPMUL_ENGINE_IMAD && engine != MPMUL_ENGINE_TENSOR) return MPDIV_ERR_BAD_ARG;
     if (!a || !b || !c || a_limbs <= 0 || b_limbs <= 0 || c_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
     if ((a_limbs | b_limbs | c_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (!aligned16(a) || !aligned16(b) || !aligned16(c)) return MPDIV_ERR_BAD_ARG;
@@ -221,6 +291,7 @@ int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, 
     if (a_limbs > MPDIV_MAX_LIMBS || b_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (engine == MPMUL_ENGINE_TENSOR) return launch_mul<512>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st, true);
     const int big = a_limbs > b_limbs ? a_limbs : b_limbs;
     switch (threads_for(big)) {
         case 64: return launch_mul<64>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st);

@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(T, 512 / T)
 shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
              DivLayout L, int clip)
 {
-    extern __shared__ __align__(16) uint32_t smem[];
+    extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;
     Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
     const ShinvBufs bufs = refine_bufs(smem, L);
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(T, 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip)
 {
-    extern __shared__ __align__(16) uint32_t smem[];
+    extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
     limb *U = smem + L.u_off;          // dividend at U + 4 (same)
     limb *WA = smem + L.wa_off;        // shinv, then the quotient

@@ -74,6 +74,50 @@ def test_mul_parity(an, bn, cn):
     assert bad.size == 0, "instances %s differ" % bad[:8]
 
 
+@pytest.mark.parametrize("an,bn,cn", [
+    (1024, 1024, 2048), (2048, 2048, 4096), (4096, 4096, 8192), (4096, 4096, 4096), (8192, 4096, 4132),
+    (32, 32, 64), (100, 36, 136), (36, 1000, 1036), (4096, 4100, 8196), (2052, 2080, 4132), (8192, 4096, 8192),
+])
+def test_mul_tensor_engine_parity(an, bn, cn):
+    """The int8 tcgen05 engine (csrc/mp_mma.cuh) must give the same limbs as the schoolbook oracle."""
+    batch = 10
+    rng = inputs.rng_for(210, an % 65536)
+    a = inputs._uniform(rng, batch, an)
+    b = inputs._uniform(rng, batch, bn)
+    a[1, an // 2:] = 0
+    b[2, max(1, bn // 3):] = 0
+    a[3, :] = 0xFFFFFFFF                      # largest byte-column sums and longest carry chains
+    b[3, :] = 0xFFFFFFFF
+    a[4, :] = 0
+    b[5, 1:] = 0
+    a[6, :] = 0xFFFFFFFF
+    b[6, :] = 0
+    b[6, 0] = 1
+    binding.debug_counters(reset=True)
+    c = host(binding.mpmul_batch(dev(a), dev(b), cn, engine=binding.ENGINE_TENSOR))
+    co = oracle.mul_batch(a, b, cn)
+    bad = np.nonzero((c != co).any(axis=1))[0]
+    assert bad.size == 0, "instances %s differ" % bad[:8]
+    assert binding.debug_counters(reset=True)["mma_wait_failures"] == 0
+
+
+def test_mul_tensor_engine_refuses_what_does_not_fit():
+    a = torch.zeros((1, 8192), dtype=torch.int32, device="cuda")
+    with pytest.raises(binding.MpdivError) as e:
+        binding.mpmul_batch(a, a, 16384, engine=binding.ENGINE_TENSOR)     # 512 blocks fit TMEM, not shared memory
+    assert e.value.code == binding.ERR_UNSUPPORTED
+
+
+def test_div_uses_tensor_engine_at_2_18_bits():
+    """Config 4 must really run its large range products on the tensor core (and get the oracle's answer:
+    test_div_config_full_size checks that)."""
+    u, v = inputs.config(4, batch=8)
+    binding.debug_counters(reset=True)
+    gpu_div(u, v)
+    cnt = binding.debug_counters(reset=True)
+    assert cnt["mma_products"] >= 2 * 8 and cnt["mma_wait_failures"] == 0
+
+
 # ------------------------------------------------------------------ shifted inverse
 @pytest.mark.parametrize("vn,h", [(4, 7), (8, 16), (16, 17), (64, 128), (512, 1024), (1024, 2048),
                                   (260, 777), (2048, 4096), (4096, 8192), (512, 512), (512, 300)])
