@@ -38,6 +38,22 @@ struct Blk {
 // ---------------------------------------------------------------------------------------
 // block collectives
 // ---------------------------------------------------------------------------------------
+// Every primitive is a template on T = the number of threads that take part.  T = 32 is the "narrow"
+// form: warp 0 of a larger block runs the operation alone (the early Newton iterations, whose operands
+// are a few tiles long), the group barrier is a __syncwarp and the other warps neither spend issue slots
+// nor meet a block barrier.
+template <int T>
+__device__ __forceinline__ void grp_sync()
+{
+    if (T == 32) __syncwarp();
+    else __syncthreads();
+}
+template <int T>
+__device__ __forceinline__ bool grp_or(bool pred)
+{
+    if (T == 32) return __any_sync(0xffffffffu, pred) != 0;
+    return __syncthreads_or(pred) != 0;
+}
 template <int T>
 __device__ __forceinline__ int block_max(int v, Blk &blk)
 {
@@ -47,7 +63,7 @@ __device__ __forceinline__ int block_max(int v, Blk &blk)
     volatile uint32_t *code = blk.sc->code[blk.parity & 1];
     blk.parity++;
     if (lane == 0) code[warp] = (uint32_t)v;
-    __syncthreads();
+    grp_sync<T>();
     int r = (lane < NW) ? (int)code[lane] : INT32_MIN;
     return __reduce_max_sync(0xffffffffu, r);
 }
@@ -69,7 +85,7 @@ __device__ __forceinline__ uint32_t carry_scan(uint32_t g, uint32_t p, uint32_t 
     volatile uint32_t *code = blk.sc->code[blk.parity & 1];
     blk.parity++;
     if (lane == 0) code[warp] = wg | wp;
-    __syncthreads();
+    grp_sync<T>();
     const uint32_t c = (lane < NW) ? code[lane] : 0u;
     const uint64_t GW = __ballot_sync(0xffffffffu, (c & 1u) != 0);
     const uint64_t PW = __ballot_sync(0xffffffffu, (c & 2u) != 0);
@@ -210,7 +226,7 @@ __device__ __forceinline__ uint32_t lin_addsub(limb *dst, int len, FA fa, FB fb,
         }
         cin = cout;
     }
-    __syncthreads();
+    grp_sync<T>();
     return cin;
 }
 
@@ -246,14 +262,14 @@ __device__ __forceinline__ void lin_copy(limb *dst, int len, const limb *src, in
         const int j = i + off;
         dst[i] = (j >= 0 && j < n) ? src[j] : 0u;
     }
-    __syncthreads();
+    grp_sync<T>();
 }
 
 template <int T>
 __device__ __forceinline__ void lin_zero(limb *dst, int len)
 {
     for (int i = threadIdx.x; i < len; i += T) dst[i] = 0u;
-    __syncthreads();
+    grp_sync<T>();
 }
 
 // any limb of a[lo, hi) non-zero?  (block-uniform result)
@@ -262,7 +278,7 @@ __device__ __forceinline__ bool any_nonzero(const limb *a, int lo, int hi)
 {
     uint32_t acc = 0;
     for (int i = lo + (int)threadIdx.x; i < hi; i += T) acc |= a[i];
-    return __syncthreads_or(acc != 0) != 0;
+    return grp_or<T>(acc != 0);
 }
 
 // number of significant limbs of a[0, n)  ("prec")

@@ -105,11 +105,120 @@ __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na,
     return -1;
 }
 
+// One Refine iteration (Alg. 1 lines 19-25 with Step and PowDiff inlined) run by a group of TT threads:
+// the whole block (TT = T) or, for the early iterations whose operands are a few tiles long, warp 0 alone
+// (TT = 32: warp-level barriers only; the other warps wait at the block barrier that ends the narrow phase
+// and leave their issue slots to the other blocks of the SM).
+template <int TT>
+__device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it, int l, int wlen, limb *Wc, limb *Wn,
+                                            limb *X, limb *P, const MulScratch &ms, Blk &blk, bool clip, MmaCtx *mma)
+{
+    const int g = 2;
+    const int m = min(H + 1 - l, l);
+    int s = max(0, k - 2 * l + 1 - g);
+    s &= ~3;                                               // keep the divisor prefix 16-byte aligned
+    const limb *Vp = V + s;                                // shift_{-s}(v)
+    const int pv = k + 1 - s;
+    const int hp = k + l + m - s + g;                      // h' of Step
+    const int hpp = hp - m;                                // h'' of PowDiff
+    const int pw = top_prec(Wc, min(wlen, l + g + 2));
+    const int d = hp - 2 * m;                              // limbs of w*x that shift_{2m-h'} drops
+
+    // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
+    const int L = pv + pw - (l - g) + 1;
+    bool positive;
+    int xl;                                                // limbs of x (upper bound)
+    int c = 0;                                             // X holds x / B^c
+    if (L >= hpp) {
+        // no room to truncate: full product and a comparison with B^h''
+        mul_full<TT>(Vp, pv, Wc, pw, P, ms, blk);
+        const int pl = round_up(pv, TILE) + round_up(pw, TILE);
+        positive = !any_nonzero<TT>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
+        if (positive) {
+            xl = hpp;                                      // x = B^h'' - p = ~p + 1 over h'' limbs
+            lin_addsub<TT, false>(X, round_up(xl, TILE), NotView{P, xl, pl}, ZeroView{}, 1u, blk);
+            // p = 0 cannot happen (v', w > 0); p = B^h'' exactly falls in the other branch
+        } else {
+            xl = pv + pw;                                  // x = p - B^h''
+            lin_addsub<TT, true>(X, round_up(xl, TILE), LimbView{P, pl, 0}, UnitView{hpp}, 0u, blk);
+        }
+    } else {
+        // c_x: x must be right down to limb c_x for w*x to be right down to limb d + 1
+        const int cx = d + 1 - pw;
+        const int Klo2 = (clip && cx >= 25) ? (cx - 9) / 8 - 1 : 0;
+        if (Klo2 <= 0) {
+            // close product: only the L low limbs of v'w (MULTMOD)
+            mul_low<TT>(Vp, pv, Wc, pw, L, P, ms, blk);
+            positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
+            xl = L;
+            if (positive)
+                lin_addsub<TT, false>(X, round_up(xl, TILE), NotView{P, xl, xl}, ZeroView{}, 1u, blk);
+            else
+                lin_copy<TT>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
+        } else {
+            // clipped close product: limbs [c, L) of v'w only; X holds x / B^c (low limbs taken as 0)
+            count(CNT_CLIPPED_STEPS);
+            const int dlo = (cx - 1) / 32;               // tensor-core form: blocks of 32 limbs, E < B^(32 dlo + 1)
+            if (try_mma_range<TT>(mma, Vp, pv, Wc, pw, dlo, (L + 31) / 32, P, ms.HI, blk) >= 0) {
+                c = 32 * dlo;
+                count(CNT_MMA_PRODUCTS);
+            } else {
+                c = TILE * Klo2;
+                mul_range<TT>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
+            }
+            xl = L - c;
+            positive = P[xl - 1] != 0u;
+            for (int i = threadIdx.x; i < round_up(xl, TILE); i += TT)
+                X[i] = (i < xl) ? (positive ? ~P[i] : P[i]) : 0u;
+            grp_sync<TT>();
+        }
+    }
+    if (!positive) count(CNT_SIGN_NEG);
+    xl = top_prec(X, xl);
+    PHASE(16 + (it & 15));
+
+    // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
+    const int nlen = round_up(l + m + g + 2, TILE);
+    if (xl == 0) {
+        lin_copy<TT>(Wn, nlen, Wc, wlen, 1 - m);
+    } else {
+        // w*x / B^(d+1): the shift_{2m-h'} of Step and the shift_{-1} of Refine drop d + 1 limbs
+        const int dd = d + 1 - c;
+        const int Klo1 = (clip && dd >= 17) ? (dd - 9) / TILE : 0;
+        int tl = -1, off = 0;
+        bool exact = (Klo1 == 0 && c == 0);
+        if (clip && dd >= 33) {
+            const int dlo = (dd - 1) / 32;
+            tl = try_mma_range<TT>(mma, Wc, pw, X, xl, dlo, 1 << 20, P, ms.HI, blk);
+            if (tl >= 0) { off = dd - 32 * dlo; exact = false; count(CNT_MMA_PRODUCTS); }
+        }
+        if (tl >= 0) {
+        } else if (Klo1 == 0) {
+            mul_full<TT>(Wc, pw, X, xl, P, ms, blk);
+            tl = round_up(pw, TILE) + round_up(xl, TILE);
+            off = dd;
+        } else {
+            tl = mul_range<TT>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
+            off = dd - TILE * Klo1;
+        }
+        if (positive) {
+            lin_addsub<TT, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, 0u, blk);
+        } else {
+            // floor of a negative: borrow one when any dropped limb of w*x is non-zero (exact path only;
+            // a clipped step is off by less than a guard-limb unit either way)
+            uint32_t bin = 0u;
+            if (exact) bin = any_nonzero<TT>(P, 0, min(dd, tl)) ? 1u : 0u;
+            lin_addsub<TT, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
+        }
+    }
+    PHASE(32 + (it & 15));
+}
+
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
-                                           bool clip, MmaCtx *mma = nullptr)
+                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
     const MulScratch &ms = bufs.ms;
@@ -154,105 +263,24 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
 
     // ---- Refine (Alg. 1 lines 15-28) ------------------------------------------------------------
     PHASE(0);
+    // The early iterations (l <= NARROW_L: operands of at most ~40 x 70 limbs) run on warp 0 alone.
+    // (narrow_l = 33 when the grid has more blocks than SMs: a lone block per SM is latency bound and keeps all
+    // its threads; 0 disables)
+    bool narrow_open = false;
     for (int it = 0; it < iters; ++it) {
         const int m = min(H + 1 - l, l);
-        int s = max(0, k - 2 * l + 1 - g);
-        s &= ~3;                                               // keep the divisor prefix 16-byte aligned
-        const limb *Vp = V + s;                                // shift_{-s}(v)
-        const int pv = k + 1 - s;
-        const int hp = k + l + m - s + g;                      // h' of Step
-        const int hpp = hp - m;                                // h'' of PowDiff
-        const int pw = top_prec(Wc, min(wlen, l + g + 2));
-        const int d = hp - 2 * m;                              // limbs of w*x that shift_{2m-h'} drops
-
-        // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
-        const int L = pv + pw - (l - g) + 1;
-        bool positive;
-        int xl;                                                // limbs of x (upper bound)
-        int c = 0;                                             // X holds x / B^c
-        if (L >= hpp) {
-            // no room to truncate: full product and a comparison with B^h''
-            mul_full<T>(Vp, pv, Wc, pw, P, ms, blk);
-            const int pl = round_up(pv, TILE) + round_up(pw, TILE);
-            positive = !any_nonzero<T>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
-            if (positive) {
-                xl = hpp;                                      // x = B^h'' - p = ~p + 1 over h'' limbs
-                lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, pl}, ZeroView{}, 1u, blk);
-                // p = 0 cannot happen (v', w > 0); p = B^h'' exactly falls in the other branch
-            } else {
-                xl = pv + pw;                                  // x = p - B^h''
-                lin_addsub<T, true>(X, round_up(xl, TILE), LimbView{P, pl, 0}, UnitView{hpp}, 0u, blk);
-            }
-        } else {
-            // c_x: x must be right down to limb c_x for w*x to be right down to limb d + 1
-            const int cx = d + 1 - pw;
-            const int Klo2 = (clip && cx >= 25) ? (cx - 9) / 8 - 1 : 0;
-            if (Klo2 <= 0) {
-                // close product: only the L low limbs of v'w (MULTMOD)
-                mul_low<T>(Vp, pv, Wc, pw, L, P, ms, blk);
-                positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
-                xl = L;
-                if (positive)
-                    lin_addsub<T, false>(X, round_up(xl, TILE), NotView{P, xl, xl}, ZeroView{}, 1u, blk);
-                else
-                    lin_copy<T>(X, round_up(xl, TILE), P, xl, 0);  // v'w = B^h'' + P, P small (or P = 0)
-            } else {
-                // clipped close product: limbs [c, L) of v'w only; X holds x / B^c (low limbs taken as 0)
-                count(CNT_CLIPPED_STEPS);
-                const int dlo = (cx - 1) / 32;               // tensor-core form: blocks of 32 limbs, E < B^(32 dlo + 1)
-                if (try_mma_range<T>(mma, Vp, pv, Wc, pw, dlo, (L + 31) / 32, P, ms.HI, blk) >= 0) {
-                    c = 32 * dlo;
-                    count(CNT_MMA_PRODUCTS);
-                } else {
-                    c = TILE * Klo2;
-                    mul_range<T>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
-                }
-                xl = L - c;
-                positive = P[xl - 1] != 0u;
-                for (int i = threadIdx.x; i < round_up(xl, TILE); i += T)
-                    X[i] = (i < xl) ? (positive ? ~P[i] : P[i]) : 0u;
-                __syncthreads();
-            }
-        }
-        if (!positive) count(CNT_SIGN_NEG);
-        xl = top_prec(X, xl);
-        PHASE(16 + (it & 15));
-
-        // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
         const int nlen = round_up(l + m + g + 2, TILE);
-        if (xl == 0) {
-            lin_copy<T>(Wn, nlen, Wc, wlen, 1 - m);
+        if (T > 32 && l <= narrow_l && it + 2 < iters) {
+            narrow_open = true;
+            if (threadIdx.x < 32) refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, nullptr);
         } else {
-            // w*x / B^(d+1): the shift_{2m-h'} of Step and the shift_{-1} of Refine drop d + 1 limbs
-            const int dd = d + 1 - c;
-            const int Klo1 = (clip && dd >= 17) ? (dd - 9) / TILE : 0;
-            int tl = -1, off = 0;
-            bool exact = (Klo1 == 0 && c == 0);
-            if (clip && dd >= 33) {
-                const int dlo = (dd - 1) / 32;
-                tl = try_mma_range<T>(mma, Wc, pw, X, xl, dlo, 1 << 20, P, ms.HI, blk);
-                if (tl >= 0) { off = dd - 32 * dlo; exact = false; count(CNT_MMA_PRODUCTS); }
+            if (narrow_open) {                                 // leave the narrow phase: one block barrier,
+                narrow_open = false;                           // and a common collective parity again
+                __syncthreads();
+                blk.parity = 0;
             }
-            if (tl >= 0) {
-            } else if (Klo1 == 0) {
-                mul_full<T>(Wc, pw, X, xl, P, ms, blk);
-                tl = round_up(pw, TILE) + round_up(xl, TILE);
-                off = dd;
-            } else {
-                tl = mul_range<T>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
-                off = dd - TILE * Klo1;
-            }
-            if (positive) {
-                lin_addsub<T, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, 0u, blk);
-            } else {
-                // floor of a negative: borrow one when any dropped limb of w*x is non-zero (exact path only;
-                // a clipped step is off by less than a guard-limb unit either way)
-                uint32_t bin = 0u;
-                if (exact) bin = any_nonzero<T>(P, 0, min(dd, tl)) ? 1u : 0u;
-                lin_addsub<T, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
-            }
+            refine_step<T>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, mma);
         }
-        PHASE(32 + (it & 15));
         l = l + m - 1;
         wlen = nlen;
         limb *t = Wc; Wc = Wn; Wn = t;

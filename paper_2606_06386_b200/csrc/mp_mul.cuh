@@ -288,7 +288,7 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
             OV[K] = d[16];
         }
     }
-    __syncthreads();
+    grp_sync<T>();
     return tiles;
 }
 
@@ -322,7 +322,7 @@ __device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, l
             c3 += inc8(s, ov);
             C3[K] = c3;
         }
-        __syncthreads();
+        grp_sync<T>();
         uint32_t g = 0, p = 0;
         if (active) {
             const uint32_t cprev = (K > Klo) ? C3[K - 1] : 0u;
@@ -339,7 +339,7 @@ __device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, l
         }
         cin = cout;
     }
-    __syncthreads();
+    grp_sync<T>();
     return blk.parity;
 }
 

@@ -84,7 +84,7 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
 template <int T>
 __global__ void __launch_bounds__(T, 512 / T)
 shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ w, int w_limbs, int batch,
-             DivLayout L, int clip)
+             DivLayout L, int clip, int narrow_l)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;
@@ -109,9 +109,9 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
             count(CNT_ONE_LIMB);
             if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }   // v*B at the (aligned) base V
             __syncthreads();
-            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0);
+            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0, nullptr, narrow_l);
         } else {
-            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0);
+            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0, nullptr, narrow_l);
         }
         store_number<T>(wout, bufs.WA, w_limbs, round_up(nw, TILE));
         __syncthreads();
@@ -125,7 +125,7 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 template <int T>
 __global__ void __launch_bounds__(T, 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
-             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip)
+             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
@@ -196,7 +196,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
         PHASE(1);
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma);
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l);
         const int psh = top_prec(WA, nw);
         PHASE(2);
 
@@ -320,6 +320,10 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 // ---------------------------------------------------------------------------------------
 namespace {
 
+// Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
+// give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
+int narrow_for(int batch) { return batch > g_sm_count ? 33 : 0; }
+
 template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
                cudaStream_t st, int clip)
@@ -329,7 +333,7 @@ int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, 
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip);
+    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(batch));
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
@@ -353,7 +357,7 @@ int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int ba
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(shinv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
-    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L, clip);
+    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L, clip, narrow_for(batch));
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
