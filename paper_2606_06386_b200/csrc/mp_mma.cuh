@@ -214,10 +214,11 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
 // to the size of the full product.  All T threads call it; ends with the result visible to the block.
 // Returns the number of limbs stored, or -1 when the request does not fit (TMEM columns or row buffer).
 template <int T>
-__device__ __noinline__ int mma_mul_range(MmaCtx &cx, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
+__device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
                                           limb *P, limb *HI, Blk &blk)
 {
     static_assert(T >= 128 && T % 32 == 0, "four epilogue warps and an issuer");
+    MmaCtx cx = cx_mem;        // work on a register copy: the asm memory clobbers would reload every field
     const int tid = threadIdx.x, warp = tid >> 5;
     const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
     dhi = min(dhi, (na + nb + 31) / 32);
@@ -322,6 +323,9 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx, const limb *A, int na, con
     // ---- P += HI with block-wide carry propagation (the carry out of the top block is dropped: mod B^(32 dhi)) ----
     lin_addsub<T, false>(P, 32 * N, LimbView{P, 32 * N, 0}, LimbView{HI, 32 * N, 0}, 0u, blk);
     MMA_T(4);
+    cx_mem.it = cx.it;
+    cx_mem.ndone = cx.ndone;
+    cx_mem.fail = cx.fail;
     return 32 * N;
 }
 
