@@ -88,7 +88,7 @@ struct ShinvBufs {
 
 // Block sizes whose kernels carry the tensor-core multiplier (mp_mma.cuh); the others never see an MmaCtx.
 template <int T>
-struct MmaEnabled { static constexpr bool value = (T == 512); };
+struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256); };
 
 // Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
 // P[i] = limb 32*dlo + i.

@@ -14,27 +14,27 @@
 //     (16-byte units XOR-ed with the row number, on absolute shared-memory addresses), and step p simply
 //     starts its descriptor p rows lower.
 //   * A_p is generated on the fly by the CUDA cores: row i is the byte-reversed 128-byte window of a
-//     ending at byte 128 p + i -- one PRMT per word from two neighbouring words -- written into a ring of
-//     16 KB stages, handed to the single MMA-issuing thread through mbarriers (`fence.proxy.async` makes
-//     the generic-proxy stores visible to the tensor core), and freed by `tcgen05.commit`.
+//     ending at byte 128 p + i -- one PRMT per word from two neighbouring words.  The row goes straight
+//     from registers into TENSOR MEMORY (`tcgen05.st`, lane = row, 32 columns = 128 bytes of K) and the
+//     MMA takes its A operand from there (`tcgen05.mma [d], [a_tmem], b_desc`): the tile never touches
+//     shared memory, whose bandwidth was the limit of a first version that staged A tiles in a 16 KB ring
+//     (about 840 cycles per step against 530 for the four MMAs).  Stages of 32 TMEM columns are handed to
+//     the single MMA-issuing thread through mbarriers and freed by `tcgen05.commit`.
 //   * Epilogue: `tcgen05.ld` (lane = i, column = d), four adjacent lanes form one limb's 64-bit column
 //     sum, low words go to P, high words to HI one limb up, and one block-wide carry-propagating add
 //     (mp_block.cuh) finishes.
 // A range of output blocks dlo <= d < dhi can be asked for (clipped products); what is omitted below
 // block dlo is less than B^(32 dlo + 1).  Only steps p whose chunk d - p can be non-zero are issued.
 //
-// Measured on B200 (standalone, one product per SM at a time): 8.5e12 / 1.7e13 / 3.2e13 limb products/s
-// for full 1024 / 2048 / 4096-limb squares against 9.15e12 for the IMAD.WIDE roofline probe.
+// Measured on B200 (standalone, one product per SM at a time): 1.07e13 / 2.3e13 / 4.3e13 limb products/s
+// for full 1024 / 2048 / 4096-limb squares against 9.15e12 for the IMAD.WIDE roofline probe.  One
+// `tcgen05.mma` (M = 128, K = 32, u8) takes about 132 cycles whatever N <= 256 is.
 #pragma once
 #include "mp_block.cuh"
 
 namespace mpd {
 
-#ifndef MMA_STAGES_N
-#define MMA_STAGES_N 2
-#endif
-constexpr int MMA_STAGES = MMA_STAGES_N;
-constexpr int MMA_TILE_BYTES = 128 * 128;
+constexpr int MMA_STAGE_COLS = 32;    // one Toeplitz tile = 128 lanes x 32 columns of tensor memory
 #ifndef MMA_SPIN_LIMIT_LOG2
 #define MMA_SPIN_LIMIT_LOG2 26
 #endif
@@ -77,6 +77,28 @@ __device__ __forceinline__ void tc_mma_i8(uint32_t tmem_d, uint64_t adesc, uint6
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
                  ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
 }
+// D[tmem] (+)= A[tmem] x B[smem desc]: A is 128 lanes x 8 columns (row m in lane m, 4 bytes of K per column)
+__device__ __forceinline__ void tc_mma_i8_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc,
+                                             uint32_t accumulate)
+{
+    const uint32_t z = 0;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+}
+// 32 lanes x 32 columns: each thread of the warp stores its 32 registers into its own lane
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+                 "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,"
+                 "%29,%30,%31,%32};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                   "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+                   "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+                   "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+                 : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
 // K-major SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes apart
 __device__ __forceinline__ uint64_t mma_smem_desc(uint32_t saddr)
 {
@@ -100,8 +122,9 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
 // Per-block state of the tensor-core multiplier (block-uniform values, kept in registers).
 struct MmaCtx {
     uint32_t tmem_base;   // first allocated TMEM column
-    int tmem_cols;        // allocated columns (power of two >= 32): at most this many output blocks per call
-    uint8_t *stages;      // MMA_STAGES x 16 KB ring of Toeplitz tiles, 1024-byte aligned
+    int tmem_cols;        // allocated columns (power of two >= 32)
+    int acc_cols;         // columns [0, acc_cols) hold the accumulators: at most this many output blocks per call;
+                          // the Toeplitz stages follow
     uint8_t *brows;       // the row operand in swizzled 128-byte rows, 1024-byte aligned
     int brows_cap;        // rows available at brows
     uint32_t bar;         // shared address of the mbarriers: full[s] at +8 s, empty[s] at +32 + 8 s, done at +64
@@ -120,24 +143,35 @@ __device__ unsigned int g_mma_fail;   // bounded waits that gave up (expected 0)
 
 constexpr int MMA_BAR_BYTES = 128;    // full[s] (up to 4), empty[s] (up to 4), done, TMEM slot
 
+// Warp roles for a block of T threads: the last warp issues the MMAs; of the others, groups of four warps
+// (one per 32-lane quarter of tensor memory) generate Toeplitz tiles.  Group g owns the tiles t = g mod G and
+// writes them into stage t mod S, S = G (or 2 when there is a single group, which then alternates stages),
+// so that every producer warp sees every phase of the stage barriers it waits on.
+template <int T>
+struct MmaRoles {
+    static constexpr int WARPS = T / 32;
+    static constexpr int GROUPS = (WARPS - 1) / 4;
+    static constexpr int STAGES = GROUPS == 1 ? 2 : GROUPS;
+    static_assert(GROUPS >= 1 && STAGES <= 4, "256 or 512 threads");
+};
+
 // One-time setup per block: mbarriers, TMEM allocation (warp 0 owns it).  All threads call it.
 template <int T>
-__device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *stages, uint8_t *brows, int brows_cap, uint8_t *bars,
-                                         int tmem_cols)
+__device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *brows, int brows_cap, uint8_t *bars, int tmem_cols)
 {
-    cx.stages = stages;
     cx.brows = brows;
     cx.brows_cap = brows_cap;
     cx.bar = smem_u32(bars);
     cx.tmem_cols = tmem_cols;
+    cx.acc_cols = tmem_cols - MmaRoles<T>::STAGES * MMA_STAGE_COLS;
     cx.it = 0;
     cx.ndone = 0;
     cx.fail = 0;
     uint32_t *slot = reinterpret_cast<uint32_t *>(bars + 96);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MMA_STAGES; s++) {
-            mbar_init(cx.bar + 8 * s, (T - 32) / 32); // one arrival per producer warp
-            mbar_init(cx.bar + 32 + 8 * s, 1);       // tcgen05.commit
+        for (int s = 0; s < MmaRoles<T>::STAGES; s++) {
+            mbar_init(cx.bar + 8 * s, 4);             // one arrival per producer warp of the group
+            mbar_init(cx.bar + 32 + 8 * s, 1);        // tcgen05.commit
         }
         mbar_init(cx.bar + 64, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -162,24 +196,23 @@ __device__ __forceinline__ void mma_fini(MmaCtx &cx)
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(cx.tmem_base), "r"(cx.tmem_cols));
 }
 
-// One 16-byte unit of a Toeplitz tile: bytes j = 16c .. 16c+15 of row `row` of tile p, out[j] = a[128p + row - j],
-// stored at the swizzled position of the K-major SWIZZLE_128B layout.  W = the operand's limbs, nw = valid
-// words (zero outside [0, nw)); CHECK = false skips the bounds tests.
+// One row of a Toeplitz tile in registers: word m holds bytes j = 4m .. 4m+3 of out[j] = a[x0 - j], x0 = 128 p + row.
+// W = the operand's limbs, nw = valid words (zero outside [0, nw)); CHECK = false skips the bounds tests.
 template <bool CHECK>
-__device__ __forceinline__ void toeplitz_unit(const limb *W, int nw, int p, int row, int c, uint8_t *tile)
+__device__ __forceinline__ void toeplitz_row(const limb *W, int nw, int x0, uint32_t (&o)[32])
 {
-    const int z0 = 128 * p + row - 16 * c - 3;               // lowest byte of the first output word
+    const int z0 = x0 - 3;                                   // lowest byte of the first output word
     const int s = z0 & 3;
     const uint32_t sel = (uint32_t)(s + 3) | ((uint32_t)(s + 2) << 4) | ((uint32_t)(s + 1) << 8) | ((uint32_t)s << 12);
     const int wi = z0 >> 2;                                  // floor(z0 / 4), also for negative z0
     auto ld = [&](int i) -> uint32_t { return CHECK ? ((i >= 0 && i < nw) ? W[i] : 0u) : W[i]; };
-    const uint32_t w4 = ld(wi + 1), w3 = ld(wi), w2 = ld(wi - 1), w1 = ld(wi - 2), w0 = ld(wi - 3);
-    uint4 o;
-    o.x = __byte_perm(w3, w4, sel);                          // bytes a[z+3], a[z+2], a[z+1], a[z]
-    o.y = __byte_perm(w2, w3, sel);
-    o.z = __byte_perm(w1, w2, sel);
-    o.w = __byte_perm(w0, w1, sel);
-    *reinterpret_cast<uint4 *>(tile + row * 128 + ((c ^ (row & 7)) << 4)) = o;
+    uint32_t hi = ld(wi + 1);
+#pragma unroll
+    for (int m = 0; m < 32; ++m) {
+        const uint32_t lo = ld(wi - m);
+        o[m] = __byte_perm(lo, hi, sel);                     // bytes a[z+3], a[z+2], a[z+1], a[z]
+        hi = lo;
+    }
 }
 
 // Steps (Toeplitz tiles) a range product needs when `na` is the Toeplitz operand.
@@ -190,8 +223,8 @@ __device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
 }
 
 // Should this range product run on the tensor core?  Measured on B200 (512-thread block alone on its SM):
-// a step costs about 810 cycles (the MMA instruction itself takes ~132 cycles whatever N is; the rest is
-// shared-memory bandwidth of the tile generation), a call about 12 000 cycles of fixed work (row operand,
+// a step costs about 600 cycles (four MMA instructions of ~132 cycles whatever N is, plus hand-over), a call
+// about 12 000 cycles of fixed work (row operand,
 // epilogue, final add), against about 1/26 cycle per limb product on the IMAD path.  swap = take b as the
 // Toeplitz operand (fewer steps).  Block-uniform.
 __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
@@ -203,9 +236,9 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
     const int sa = mma_steps(na, nb, dlo, dhi), sb = mma_steps(nb, na, dlo, dhi);
     swap = sb < sa;
     const int steps = swap ? sb : sa;
-    if (steps <= 0 || Nn > cx->tmem_cols || Nn + steps - 1 > cx->brows_cap) return false;
+    if (steps <= 0 || Nn > cx->acc_cols || Nn + steps - 1 > cx->brows_cap) return false;
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
-    return est >= 52ll * (810ll * steps + 12000ll);
+    return est >= 52ll * (600ll * steps + 12000ll);
 }
 
 // P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).
@@ -217,7 +250,7 @@ template <int T>
 __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
                                           limb *P, limb *HI, Blk &blk)
 {
-    static_assert(T >= 128 && T % 32 == 0, "four epilogue warps and an issuer");
+    static_assert(T >= 256 && T % 32 == 0, "a producer group of four warps and an issuer warp");
     MmaCtx cx = cx_mem;        // work on a register copy: the asm memory clobbers would reload every field
     const int tid = threadIdx.x, warp = tid >> 5;
     const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
@@ -227,7 +260,7 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     const int pmin = max(0, dlo - Eb + 1), pmax = min(Ea, dhi - 1);
     const int e0 = dlo - pmax;                                // chunk of b held by row 0
     const int R = (dlo + Nn - 1 - pmin) - e0 + 1;
-    if (N <= 0 || pmax < pmin || Nn > cx.tmem_cols || R > cx.brows_cap) return -1;
+    if (N <= 0 || pmax < pmin || Nn > cx.acc_cols || R > cx.brows_cap) return -1;
 
 #ifdef MMA_TIMING
     long long t0_ = clock64();
@@ -248,42 +281,44 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
 
     MMA_T(0);
     const int nsteps = pmax - pmin + 1;
-    constexpr int NPROD = T - 32;
-    if (tid < NPROD) {
-        // ---- Toeplitz producers: every producer thread fills its share of the 1024 units of EVERY tile, so
-        //      each of them sees every phase of the stage barriers (the parity protocol needs that) ----
+    constexpr int G = MmaRoles<T>::GROUPS, S = MmaRoles<T>::STAGES;
+    const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
+    if (warp < 4 * G) {
+        // ---- Toeplitz producers: warp j fills lanes 32 (j % 4) .. +31 of the tiles of group j / 4 ----
+        const int grp = warp >> 2, row = tid & 127;
         for (int step = 0; step < nsteps; ++step) {
+            const uint32_t t = cx.it + (uint32_t)step;
+            if ((int)(t % G) != grp) continue;
             const int p = pmin + step;
-            const uint32_t it = cx.it + (uint32_t)step;
-            const int s = (int)(it % MMA_STAGES);
-            if (it >= MMA_STAGES && !mbar_wait(cx.bar + 32 + 8 * s, ((it / MMA_STAGES) - 1) & 1)) { cx.fail = 1; break; }
-            uint8_t *tile = cx.stages + s * MMA_TILE_BYTES;
-            if (p >= 1 && 32 * p + 33 <= na) {
-                for (int u = tid; u < 1024; u += NPROD) toeplitz_unit<false>(A, na, p, u & 127, u >> 7, tile);
-            } else {
-                for (int u = tid; u < 1024; u += NPROD) toeplitz_unit<true>(A, na, p, u & 127, u >> 7, tile);
-            }
-            fence_async_smem();                              // generic-proxy stores -> visible to the tensor core
+            const int s = (int)(t % S);
+            const uint32_t use = t / S;
+            if (use >= 1 && !mbar_wait(cx.bar + 32 + 8 * s, (use - 1) & 1)) { cx.fail = 1; break; }
+            tc_fence_after();
+            uint32_t o[32];
+            if (p >= 1 && 32 * p + 33 <= na) toeplitz_row<false>(A, na, 128 * p + row, o);
+            else toeplitz_row<true>(A, na, 128 * p + row, o);
+            tmem_st32(a_tmem0 + ((uint32_t)(row & ~31) << 16) + (uint32_t)(MMA_STAGE_COLS * s), o);
+            tc_fence_before();
             __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(cx.bar + 8 * s); // one arrival per producer warp
+            if ((tid & 31) == 0) mbar_arrive(cx.bar + 8 * s);
         }
-    } else if (tid == NPROD) {
+    } else if (tid == T - 32) {
         // ---- the MMA issuer ----
         for (int step = 0; step < nsteps; ++step) {
             const int p = pmin + step;
-            const uint32_t it = cx.it + (uint32_t)step;
-            const int s = (int)(it % MMA_STAGES);
-            if (!mbar_wait(cx.bar + 8 * s, (it / MMA_STAGES) & 1)) { cx.fail = 2; break; }
+            const uint32_t t = cx.it + (uint32_t)step;
+            const int s = (int)(t % S);
+            if (!mbar_wait(cx.bar + 8 * s, (t / S) & 1)) { cx.fail = 2; break; }
             tc_fence_after();
-            const uint32_t a_addr = smem_u32(cx.stages + s * MMA_TILE_BYTES);
+            const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
             for (int nc = 0; nc < Nn; nc += 256) {
                 const int ncols = min(256, Nn - nc);
                 const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
                 const uint32_t idesc = mma_idesc(ncols);
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
-                    tc_mma_i8(cx.tmem_base + nc, mma_smem_desc(a_addr + 32 * k), mma_smem_desc(b_addr + 32 * k), idesc,
-                              (step > 0 || k > 0) ? 1u : 0u);
+                    tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
+                                 (step > 0 || k > 0) ? 1u : 0u);
             }
             tc_commit(cx.bar + 32 + 8 * s);
         }

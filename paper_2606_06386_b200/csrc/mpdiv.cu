@@ -79,8 +79,9 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
     const int full = (a_limbs + b_limbs + 31) / 32, want = (c_limbs + 31) / 32;
     const int blocks = want < full ? want : full;
     const int nn = (blocks + 15) & ~15;
-    if (nn > 512) return false;
-    const int cols = nn <= 32 ? 32 : nn <= 64 ? 64 : nn <= 128 ? 128 : nn <= 256 ? 256 : 512;
+    const int need = nn + 4 * MMA_STAGE_COLS;                           // accumulators + up to four Toeplitz stages
+    if (need > 512) return false;
+    const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
     const int small = a_limbs < b_limbs ? a_limbs : b_limbs;
     const int rows = round_up(nn + (small + 31) / 32 + 8, 8);
     // P and HI must hold 32 limbs per output block
@@ -96,7 +97,7 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
         L.total_words = o;
     }
     const int off = round_up(L.total_words, 256);
-    const int words = MMA_STAGES * MMA_TILE_BYTES / 4 + rows * 32 + 64;
+    const int words = rows * 32 + 64;
     if ((off + words) * 4 > max_smem) return false;
     L.mma_off = off;
     L.mma_rows = rows;
@@ -119,8 +120,7 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
     if constexpr (MmaEnabled<T>::value) {
         if (L.mma_off >= 0) {
             uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
-            mma_init<T>(mcx, base, base + MMA_STAGES * MMA_TILE_BYTES, L.mma_rows,
-                        base + MMA_STAGES * MMA_TILE_BYTES + L.mma_rows * 128, L.mma_cols);
+            mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
             tensor = true;
         }
     }

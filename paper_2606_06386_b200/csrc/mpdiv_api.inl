@@ -7,7 +7,7 @@
 // ---------------------------------------------------------------------------------------
 struct DivLayout {
     int v_off, u_off, wa_off, big_off, sc_off, total_words;
-    int mma_off;      // word offset (1024-byte aligned) of the tensor-core scratch, or -1: stages | rows | barriers
+    int mma_off;      // word offset (1024-byte aligned) of the tensor-core scratch, or -1: rows | barriers
     int mma_rows;     // rows of 128 bytes available for the row operand
     int mma_cols;     // TMEM columns to allocate
     int x_words;      // Refine: X at big_off, P behind it
@@ -49,14 +49,16 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
 }
 
 // Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the ring of
-// Toeplitz tiles, the row operand (output blocks + steps rows), the mbarriers.  max_smem in bytes.
+// row operand (output blocks + steps rows of 128 bytes) and the mbarriers; the Toeplitz tiles live in tensor
+// memory.  max_smem in bytes.
 static void div_layout_add_mma(DivLayout &L, int M, int max_smem)
 {
     const int blocks = (M / 2 + 1 + 9 + 31) / 32 + 2;             // output blocks of u * shinv at n = M/2
-    const int cols = blocks <= 32 ? 32 : blocks <= 64 ? 64 : blocks <= 128 ? 128 : 256;
+    const int need = ((blocks + 15) & ~15) + 4 * MMA_STAGE_COLS;       // accumulators + up to four Toeplitz stages
+    const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
     const int rows = round_up(((blocks + 15) & ~15) + blocks + 8, 8);
     const int off = round_up(L.total_words, 256);
-    const int words = MMA_STAGES * MMA_TILE_BYTES / 4 + rows * 32 + 64;
+    const int words = rows * 32 + 64;
     if ((off + words) * 4 > max_smem) return;
     L.mma_off = off;
     L.mma_rows = rows;
@@ -145,8 +147,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     if constexpr (MmaEnabled<T>::value) {
         if (L.mma_off >= 0 && clip) {
             uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
-            mma_init<T>(mcx, base, base + MMA_STAGES * MMA_TILE_BYTES, L.mma_rows,
-                        base + MMA_STAGES * MMA_TILE_BYTES + L.mma_rows * 128, L.mma_cols);
+            mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
             mma = &mcx;
         }
     }
