@@ -127,7 +127,7 @@ struct MmaCtx {
                           // the Toeplitz stages follow
     uint8_t *brows;       // the row operand in swizzled 128-byte rows, 1024-byte aligned
     int brows_cap;        // rows available at brows
-    uint32_t bar;         // shared address of the mbarriers: full[s] at +8 s, empty[s] at +32 + 8 s, done at +64
+    uint32_t bar;         // shared address of the mbarriers: full[s] at +8 s, empty[s] at +64 + 8 s, done at +128
     uint32_t it;          // tiles produced so far (stage index and barrier parities follow from it)
     uint32_t ndone;       // products finished so far (parity of the done barrier)
     uint32_t fail;        // set when a bounded wait gave up
@@ -141,18 +141,22 @@ __device__ unsigned long long g_mma_t[8];
 #endif
 __device__ unsigned int g_mma_fail;   // bounded waits that gave up (expected 0); reported with the debug counters
 
-constexpr int MMA_BAR_BYTES = 128;    // full[s] (up to 4), empty[s] (up to 4), done, TMEM slot
+constexpr int MMA_BAR_BYTES = 256;    // full[s] (up to 8), empty[s] (up to 8), done, TMEM slot
 
 // Warp roles for a block of T threads: the last warp issues the MMAs; of the others, groups of four warps
 // (one per 32-lane quarter of tensor memory) generate Toeplitz tiles.  Group g owns the tiles t = g mod G and
-// writes them into stage t mod S, S = G (or 2 when there is a single group, which then alternates stages),
-// so that every producer warp sees every phase of the stage barriers it waits on.
+// cycles through its own PER_GROUP stages, so that every producer warp sees every phase of the stage
+// barriers it waits on (a warp that skipped a phase would misread the parity).
 template <int T>
 struct MmaRoles {
     static constexpr int WARPS = T / 32;
     static constexpr int GROUPS = (WARPS - 1) / 4;
-    static constexpr int STAGES = GROUPS == 1 ? 2 : GROUPS;
-    static_assert(GROUPS >= 1 && STAGES <= 4, "256 or 512 threads");
+    static constexpr int PER_GROUP = GROUPS == 1 ? 4 : 2;
+    static constexpr int STAGES = GROUPS * PER_GROUP;
+    static_assert(GROUPS >= 1 && STAGES <= 6, "256 or 512 threads");
+    // stage and use count of global tile number t
+    __device__ static __forceinline__ int stage(uint32_t t) { return (int)(t % GROUPS) * PER_GROUP + (int)((t / GROUPS) % PER_GROUP); }
+    __device__ static __forceinline__ uint32_t use(uint32_t t) { return (t / GROUPS) / PER_GROUP; }
 };
 
 // One-time setup per block: mbarriers, TMEM allocation (warp 0 owns it).  All threads call it.
@@ -167,13 +171,13 @@ __device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *brows, int brows_c
     cx.it = 0;
     cx.ndone = 0;
     cx.fail = 0;
-    uint32_t *slot = reinterpret_cast<uint32_t *>(bars + 96);
+    uint32_t *slot = reinterpret_cast<uint32_t *>(bars + 144);
     if (threadIdx.x == 0) {
         for (int s = 0; s < MmaRoles<T>::STAGES; s++) {
             mbar_init(cx.bar + 8 * s, 4);             // one arrival per producer warp of the group
-            mbar_init(cx.bar + 32 + 8 * s, 1);        // tcgen05.commit
+            mbar_init(cx.bar + 64 + 8 * s, 1);        // tcgen05.commit
         }
-        mbar_init(cx.bar + 64, 1);
+        mbar_init(cx.bar + 128, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (threadIdx.x < 32) {
@@ -281,7 +285,8 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
 
     MMA_T(0);
     const int nsteps = pmax - pmin + 1;
-    constexpr int G = MmaRoles<T>::GROUPS, S = MmaRoles<T>::STAGES;
+    using Roles = MmaRoles<T>;
+    constexpr int G = Roles::GROUPS;
     const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
     if (warp < 4 * G) {
         // ---- Toeplitz producers: warp j fills lanes 32 (j % 4) .. +31 of the tiles of group j / 4 ----
@@ -290,9 +295,9 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
             const uint32_t t = cx.it + (uint32_t)step;
             if ((int)(t % G) != grp) continue;
             const int p = pmin + step;
-            const int s = (int)(t % S);
-            const uint32_t use = t / S;
-            if (use >= 1 && !mbar_wait(cx.bar + 32 + 8 * s, (use - 1) & 1)) { cx.fail = 1; break; }
+            const int s = Roles::stage(t);
+            const uint32_t use = Roles::use(t);
+            if (use >= 1 && !mbar_wait(cx.bar + 64 + 8 * s, (use - 1) & 1)) { cx.fail = 1; break; }
             tc_fence_after();
             uint32_t o[32];
             if (p >= 1 && 32 * p + 33 <= na) toeplitz_row<false>(A, na, 128 * p + row, o);
@@ -307,8 +312,8 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         for (int step = 0; step < nsteps; ++step) {
             const int p = pmin + step;
             const uint32_t t = cx.it + (uint32_t)step;
-            const int s = (int)(t % S);
-            if (!mbar_wait(cx.bar + 8 * s, (t / S) & 1)) { cx.fail = 2; break; }
+            const int s = Roles::stage(t);
+            if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) { cx.fail = 2; break; }
             tc_fence_after();
             const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
             for (int nc = 0; nc < Nn; nc += 256) {
@@ -320,9 +325,9 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
                     tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
                                  (step > 0 || k > 0) ? 1u : 0u);
             }
-            tc_commit(cx.bar + 32 + 8 * s);
+            tc_commit(cx.bar + 64 + 8 * s);
         }
-        tc_commit(cx.bar + 64);
+        tc_commit(cx.bar + 128);
     }
     cx.it += (uint32_t)nsteps;
     __syncwarp();
@@ -330,7 +335,7 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
 
     // ---- epilogue: TMEM lane i, column d  ->  byte-column sum of output byte 128 (dlo + d) + i ----
     if (warp < 4) {
-        if (!mbar_wait(cx.bar + 64, cx.ndone & 1)) cx.fail = 3;
+        if (!mbar_wait(cx.bar + 128, cx.ndone & 1)) cx.fail = 3;
         tc_fence_after();
         MMA_T(2);
         for (int d0 = 0; d0 < Nn; d0 += 16) {

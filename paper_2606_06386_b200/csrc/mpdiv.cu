@@ -79,7 +79,7 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
     const int full = (a_limbs + b_limbs + 31) / 32, want = (c_limbs + 31) / 32;
     const int blocks = want < full ? want : full;
     const int nn = (blocks + 15) & ~15;
-    const int need = nn + 4 * MMA_STAGE_COLS;                           // accumulators + up to four Toeplitz stages
+    const int need = nn + 6 * MMA_STAGE_COLS;                           // accumulators + up to six Toeplitz stages
     if (need > 512) return false;
     const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
     const int small = a_limbs < b_limbs ? a_limbs : b_limbs;

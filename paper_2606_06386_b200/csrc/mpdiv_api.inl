@@ -51,10 +51,10 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
 // Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the ring of
 // row operand (output blocks + steps rows of 128 bytes) and the mbarriers; the Toeplitz tiles live in tensor
 // memory.  max_smem in bytes.
-static void div_layout_add_mma(DivLayout &L, int M, int max_smem)
+static void div_layout_add_mma(DivLayout &L, int M, int max_smem, int stages)
 {
     const int blocks = (M / 2 + 1 + 9 + 31) / 32 + 2;             // output blocks of u * shinv at n = M/2
-    const int need = ((blocks + 15) & ~15) + 4 * MMA_STAGE_COLS;       // accumulators + up to four Toeplitz stages
+    const int need = ((blocks + 15) & ~15) + stages * MMA_STAGE_COLS;  // accumulators + the Toeplitz stages
     const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
     const int rows = round_up(((blocks + 15) & ~15) + blocks + 8, 8);
     const int off = round_up(L.total_words, 256);
@@ -321,6 +321,11 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 // ---------------------------------------------------------------------------------------
 namespace {
 
+template <int T, bool E = MmaEnabled<T>::value>
+struct MmaStagesOf { static constexpr int value = 0; };
+template <int T>
+struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; };
+
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 int narrow_for(int batch) { return batch > g_sm_count ? 33 : 0; }
@@ -330,7 +335,7 @@ int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, 
                cudaStream_t st, int clip)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem);
+    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
@@ -343,7 +348,7 @@ template <int T>
 int div_wave(int u_limbs, int v_limbs, int clip)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem);
+    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
     if (set_smem(mpdiv_kernel<T>, bytes) != MPDIV_OK) return 0;
     int nb = 0;
