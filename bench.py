@@ -38,8 +38,8 @@ W_LIMB_PRODUCTS = {1024: 1898264, 2048: 7553425, 4096: 30136284, 8192: 120394683
 IMAD_PER_CLK_PER_SM = 64
 FLUSH_BYTES = 256 << 20   # > 126 MB of L2
 
-# DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_clipped_variant.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 14739456 + 1350144, 4: 29238272 + 7290880}
+# DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_final.md)
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 15374336 + 1443584, 3: 38150144 + 15338752, 4: 37935872 + 14671872}
 
 
 def parse_args():
@@ -363,7 +363,7 @@ def run_ours(args):
             "achieved": achieved / 1e9, "peak": peak_products / 1e9, "unit": "G limb-products/s",
             "frac": achieved / peak_products, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg),
             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture per launch "
-                              "(profiles/r1_clipped_variant.md); algorithmic bytes per launch = %d" % (b * 4 * (2 * m + 2 * n)),
+                              "(profiles/r1_final.md); algorithmic bytes per launch = %d" % (b * 4 * (2 * m + 2 * n)),
             "peak_source": "measured in this run: mpdiv_imad_probe kind 0 (carry-chained IMAD.WIDE.U32 tile, no memory)",
             "nominal_imad32_peak": nominal_peak / 1e9,
             "measured_imad_lo32_peak": peaks["imad_lo32"] / 1e9,
