@@ -254,6 +254,28 @@ def test_div_random_effective_precisions_large(variant):
     check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions 2048", variant)
 
 
+@pytest.mark.parametrize("M,count", [(4096, 240), (8192, 96)])
+def test_div_random_effective_precisions_tensor_sizes(M, count):
+    """Random effective precisions at the strides whose kernels carry the tensor-core engine: every shape of
+    range product (and every decision of mma_plan) occurs, including operands far from 32-limb multiples."""
+    rng = inputs.rng_for(402, M % 65536)
+    us, vs = [], []
+    for i in range(count):
+        if i % 3 == 0:          # balanced: the shapes that do reach the tensor core
+            lu = int(rng.integers(M - 600, M + 1))
+            lv = int(rng.integers(lu // 2 - 300, lu // 2 + 300))
+        else:
+            lv = int(rng.integers(1, M + 1))
+            lu = int(rng.integers(0, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, max(1, lv)))
+    binding.debug_counters(reset=True)
+    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions %d" % M)
+    cnt = binding.debug_counters(reset=True)
+    print("counters", cnt)
+    assert cnt["mma_products"] > 0 and cnt["mma_wait_failures"] == 0 and cnt["delta_out_of_range"] == 0
+
+
 def test_div_zero_divisor_does_not_trap():
     binding.debug_counters(reset=True)
     u, v = inputs.uniform_operands(8, 64, 32, config=77)
