@@ -88,7 +88,7 @@ struct ShinvBufs {
 
 // Block sizes whose kernels carry the tensor-core multiplier (mp_mma.cuh); the others never see an MmaCtx.
 template <int T>
-struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256); };
+struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256); };   // measured: no gain at 128 threads (2^16 bits)
 
 // Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
 // P[i] = limb 32*dlo + i.
@@ -98,7 +98,7 @@ __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na,
 {
     if constexpr (MmaEnabled<T>::value) {
         bool swap;
-        if (mma_plan(mma, na, nb, dlo, dhi, swap))
+        if (mma_plan<T>(mma, na, nb, dlo, dhi, swap))
             return swap ? mma_mul_range<T>(*mma, Bp, nb, A, na, dlo, dhi, P, HI, blk)
                         : mma_mul_range<T>(*mma, A, na, Bp, nb, dlo, dhi, P, HI, blk);
     }

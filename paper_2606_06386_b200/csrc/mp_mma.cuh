@@ -150,10 +150,14 @@ constexpr int MMA_BAR_BYTES = 256;    // full[s] (up to 8), empty[s] (up to 8), 
 template <int T>
 struct MmaRoles {
     static constexpr int WARPS = T / 32;
-    static constexpr int GROUPS = (WARPS - 1) / 4;
-    static constexpr int PER_GROUP = GROUPS == 1 ? 4 : 2;
+    // 128 threads: the four warps all produce and thread 0 issues the MMAs of a step right after its own row
+    // (COMBINED); four such blocks share an SM, so each gets 128 TMEM columns: 64 accumulators + 2 stages.
+    static constexpr bool COMBINED = (WARPS == 4);
+    static constexpr int GROUPS = COMBINED ? 1 : (WARPS - 1) / 4;
+    static constexpr int PER_GROUP = COMBINED ? 2 : (GROUPS == 1 ? 4 : 2);
     static constexpr int STAGES = GROUPS * PER_GROUP;
-    static_assert(GROUPS >= 1 && STAGES <= 6, "256 or 512 threads");
+    static constexpr int ISSUER = COMBINED ? 0 : T - 32;
+    static_assert(GROUPS >= 1 && STAGES <= 6, "128, 256 or 512 threads");
     // stage and use count of global tile number t
     __device__ static __forceinline__ int stage(uint32_t t) { return (int)(t % GROUPS) * PER_GROUP + (int)((t / GROUPS) % PER_GROUP); }
     __device__ static __forceinline__ uint32_t use(uint32_t t) { return (t / GROUPS) / PER_GROUP; }
@@ -189,6 +193,14 @@ __device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *brows, int brows_c
     __syncthreads();
     tc_fence_after();
     cx.tmem_base = *slot;
+}
+
+// A kernel that CONTAINS tcgen05.alloc holds the SM's allocation permit from launch until it relinquishes it,
+// and no other block is co-scheduled on the SM meanwhile: a block that will not allocate must say so at
+// once (measured: without this, blocks that skipped mma_init ran one per SM instead of four).
+__device__ __forceinline__ void mma_decline()
+{
+    if (threadIdx.x < 32) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
 }
 
 template <int T>
@@ -231,6 +243,7 @@ __device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
 // about 12 000 cycles of fixed work (row operand,
 // epilogue, final add), against about 1/26 cycle per limb product on the IMAD path.  swap = take b as the
 // Toeplitz operand (fewer steps).  Block-uniform.
+template <int T>
 __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
 {
     if (cx == nullptr || na <= 0 || nb <= 0 || dlo < 0) return false;
@@ -242,7 +255,8 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
     const int steps = swap ? sb : sa;
     if (steps <= 0 || Nn > cx->acc_cols || Nn + steps - 1 > cx->brows_cap) return false;
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
-    return est >= 52ll * (600ll * steps + 12000ll);
+    // the IMAD path of a block of T threads gets T/512 of the SM's 26 limb products per cycle
+    return est >= (long long)(52 * T / 512) * (700ll * steps + 12000ll);
 }
 
 // P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).
@@ -254,7 +268,7 @@ template <int T>
 __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
                                           limb *P, limb *HI, Blk &blk)
 {
-    static_assert(T >= 256 && T % 32 == 0, "a producer group of four warps and an issuer warp");
+    static_assert(T >= 128 && T % 32 == 0, "a producer group of four warps");
     MmaCtx cx = cx_mem;        // work on a register copy: the asm memory clobbers would reload every field
     const int tid = threadIdx.x, warp = tid >> 5;
     const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
@@ -288,6 +302,26 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     using Roles = MmaRoles<T>;
     constexpr int G = Roles::GROUPS;
     const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
+    // the MMAs of one step: D[:, 0..Nn) += A_p x B_p (K = 128 as four instructions of K = 32)
+    auto issue_step = [&](int step) -> bool {
+        const int p = pmin + step;
+        const uint32_t t = cx.it + (uint32_t)step;
+        const int s = Roles::stage(t);
+        if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) return false;
+        tc_fence_after();
+        const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
+        for (int nc = 0; nc < Nn; nc += 256) {
+            const int ncols = min(256, Nn - nc);
+            const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
+            const uint32_t idesc = mma_idesc(ncols);
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
+                             (step > 0 || k > 0) ? 1u : 0u);
+        }
+        tc_commit(cx.bar + 64 + 8 * s);
+        return true;
+    };
     if (warp < 4 * G) {
         // ---- Toeplitz producers: warp j fills lanes 32 (j % 4) .. +31 of the tiles of group j / 4 ----
         const int grp = warp >> 2, row = tid & 127;
@@ -306,27 +340,13 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
             tc_fence_before();
             __syncwarp();
             if ((tid & 31) == 0) mbar_arrive(cx.bar + 8 * s);
+            if (Roles::COMBINED && tid == Roles::ISSUER && !issue_step(step)) { cx.fail = 2; break; }
         }
-    } else if (tid == T - 32) {
+        if (Roles::COMBINED && tid == Roles::ISSUER) tc_commit(cx.bar + 128);
+    } else if (!Roles::COMBINED && tid == Roles::ISSUER) {
         // ---- the MMA issuer ----
-        for (int step = 0; step < nsteps; ++step) {
-            const int p = pmin + step;
-            const uint32_t t = cx.it + (uint32_t)step;
-            const int s = Roles::stage(t);
-            if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) { cx.fail = 2; break; }
-            tc_fence_after();
-            const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
-            for (int nc = 0; nc < Nn; nc += 256) {
-                const int ncols = min(256, Nn - nc);
-                const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
-                const uint32_t idesc = mma_idesc(ncols);
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
-                                 (step > 0 || k > 0) ? 1u : 0u);
-            }
-            tc_commit(cx.bar + 64 + 8 * s);
-        }
+        for (int step = 0; step < nsteps; ++step)
+            if (!issue_step(step)) { cx.fail = 2; break; }
         tc_commit(cx.bar + 128);
     }
     cx.it += (uint32_t)nsteps;

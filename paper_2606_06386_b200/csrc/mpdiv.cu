@@ -122,6 +122,8 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
             uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
             mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
             tensor = true;
+        } else {
+            mma_decline();
         }
     }
 

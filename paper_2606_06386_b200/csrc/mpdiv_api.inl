@@ -149,6 +149,8 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
             mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
             mma = &mcx;
+        } else {
+            mma_decline();
         }
     }
 
