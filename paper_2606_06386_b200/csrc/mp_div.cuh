@@ -39,6 +39,10 @@ enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT
 // Phase timing for tuning builds only (-DMPDIV_PHASE_TIMING): thread 0 of block 0 accumulates the cycles
 // between consecutive PHASE() marks.  Compiles to nothing in the product build.
 #ifdef MPDIV_PHASE_TIMING
+__device__ unsigned long long g_op[16];
+#define OPDECL() long long tacc_[8] = {0,0,0,0,0,0,0,0}; long long tt_ = clock64()
+#define OPT(i) do { long long t__ = clock64(); tacc_[i] += t__ - tt_; tt_ = t__; } while (0)
+#define OPFLUSH() do { if (blockIdx.x == 0 && threadIdx.x == 0 && it < 6) for (int i_ = 0; i_ < 8; i_++) atomicAdd(&g_op[i_], (unsigned long long)tacc_[i_]); } while (0)
 __device__ unsigned long long g_phase[64];
 __device__ long long g_phase_t0;
 #define PHASE(i)                                                        \
@@ -50,6 +54,9 @@ __device__ long long g_phase_t0;
         }                                                               \
     } while (0)
 #else
+#define OPDECL() do { } while (0)
+#define OPT(i) do { } while (0)
+#define OPFLUSH() do { } while (0)
 #define PHASE(i) do { } while (0)
 #endif
 
@@ -121,7 +128,9 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     const int pv = k + 1 - s;
     const int hp = k + l + m - s + g;                      // h' of Step
     const int hpp = hp - m;                                // h'' of PowDiff
+    OPDECL(); 
     const int pw = top_prec(Wc, min(wlen, l + g + 2));
+    OPT(1);
     const int d = hp - 2 * m;                              // limbs of w*x that shift_{2m-h'} drops
 
     // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
@@ -149,6 +158,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         if (Klo2 <= 0) {
             // close product: only the L low limbs of v'w (MULTMOD)
             mul_low<TT>(Vp, pv, Wc, pw, L, P, ms, blk);
+            OPT(4);
             positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
             xl = L;
             if (positive)
@@ -174,7 +184,9 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         }
     }
     if (!positive) count(CNT_SIGN_NEG);
+    OPT(2);
     xl = top_prec(X, xl);
+    OPT(3);
     PHASE(16 + (it & 15));
 
     // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
@@ -195,6 +207,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         if (tl >= 0) {
         } else if (Klo1 == 0) {
             mul_full<TT>(Wc, pw, X, xl, P, ms, blk);
+            OPT(5);
             tl = round_up(pw, TILE) + round_up(xl, TILE);
             off = dd;
         } else {
@@ -211,6 +224,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
             lin_addsub<TT, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
         }
     }
+    OPT(7); OPFLUSH();
     PHASE(32 + (it & 15));
 }
 

@@ -124,8 +124,12 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // ---------------------------------------------------------------------------------------
 // mpdiv_batch kernel: Alg. 3, one division per block
 // ---------------------------------------------------------------------------------------
-template <int T>
-__global__ void __launch_bounds__(T, 512 / T)
+// LAT = false: 128 registers per thread, 512 threads per SM (throughput: the batch fills the SMs several
+// times over).  LAT = true: up to 255 registers, for batches that leave an SM one or two blocks -- the kernel
+// body keeps ~20 values live across the multiplier calls and spills them at 128 registers, which costs a
+// latency-bound division 20 % (config 1: 102 -> 81 us).
+template <int T, bool LAT>
+__global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l)
 {
@@ -332,17 +336,26 @@ struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; 
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 int narrow_for(int batch) { return batch > g_sm_count ? 33 : 0; }
 
-template <int T>
-int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-               cudaStream_t st, int clip)
+template <int T, bool LAT>
+int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+                 cudaStream_t st, int clip)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
-    int rc = set_smem(mpdiv_kernel<T>, bytes);
+    int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(batch));
+    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(batch));
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+template <int T>
+int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+               cudaStream_t st, int clip)
+{
+    // a batch of at most two blocks per SM is latency bound: give its threads all the registers they want
+    if (T <= 256 && batch <= 2 * g_sm_count) return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
+    return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
 }
 
 // divisions one wave of the division kernel holds on the whole GPU (blocks per SM x SMs)
@@ -352,9 +365,9 @@ int div_wave(int u_limbs, int v_limbs, int clip)
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
-    if (set_smem(mpdiv_kernel<T>, bytes) != MPDIV_OK) return 0;
+    if (set_smem(mpdiv_kernel<T, false>, bytes) != MPDIV_OK) return 0;
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mpdiv_kernel<T>, T, bytes) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mpdiv_kernel<T, false>, T, bytes) != cudaSuccess) return 0;
     return nb * g_sm_count;
 }
 
@@ -514,6 +527,10 @@ int mpdiv_debug_phases(unsigned long long out[64], int reset)
     if (cudaMemcpyFromSymbol(out, g_phase, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
     if (cudaMemcpyFromSymbol(sub, g_sub, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
     for (int i = 48; i < 64; i++) out[i] = sub[i];       // slots 48.. carry the multiplier sub-phases
+    unsigned long long op[16];
+    if (cudaMemcpyFromSymbol(op, g_op, sizeof(op)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    for (int i = 0; i < 8; i++) out[8 + i] = op[i];      // slots 8..15: op-level split of Refine iterations 0..5
+    if (reset) { unsigned long long zz[16] = {0}; cudaMemcpyToSymbol(g_op, zz, sizeof(zz)); }
     if (reset) {
         unsigned long long z[64] = {0};
         if (cudaMemcpyToSymbol(g_phase, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
