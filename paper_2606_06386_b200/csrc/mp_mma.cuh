@@ -256,7 +256,10 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
     if (steps <= 0 || Nn > cx->acc_cols || Nn + steps - 1 > cx->brows_cap) return false;
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
     // the IMAD path of a block of T threads gets T/512 of the SM's 26 limb products per cycle
-    return est >= (long long)(52 * T / 512) * (700ll * steps + 12000ll);
+#ifndef MMA_PLAN_PCT
+#define MMA_PLAN_PCT 35     // measured: the model below is pessimistic for the tensor path; 35 % is +1-2 % at 2^17, 2^18 bits
+#endif
+    return 100 * est >= (long long)(MMA_PLAN_PCT * 52 * T / 512) * (700ll * steps + 12000ll);
 }
 
 // P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).
