@@ -152,7 +152,7 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
  *   out[7] divisors that are an exact power of B (Alg. 1 line 9)
  *   out[8] 8x8-limb tile products executed (x 64 = limb products issued, tile padding included)
  *   out[9] instances needing more than one -1 step      out[10] instances whose correction loops hit
- *          their bound of 8 (result not exact; expected 0)      out[11] Newton steps that ran clipped
+ *          their bound of 64 (result not exact; expected 0)      out[11] Newton steps that ran clipped
  *   out[12] range products that ran on the tensor core (mp_mma.cuh)      out[13] bit mask of tensor-core
  *          pipeline waits that gave up (expected 0)      out[14..15] reserved (0)
  */

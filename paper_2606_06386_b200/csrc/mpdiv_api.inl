@@ -128,6 +128,10 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // times over).  LAT = true: up to 255 registers, for batches that leave an SM one or two blocks -- the kernel
 // body keeps ~20 values live across the multiplier calls and spills them at 128 registers, which costs a
 // latency-bound division 20 % (config 1: 102 -> 81 us).
+// Bound of the two correction loops of Div.  Theorem 2 needs one step; the clipped variant two or three; the
+// bound only has to keep |delta| * v below B^(k+2), the range of the remainder arithmetic.
+constexpr int CORR_MAX = 64;
+
 template <int T, bool LAT>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
@@ -287,7 +291,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             PHASE(5);
             // a11: r = u - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
             lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
-            while (R[rlen - 1] != 0u && minus < 8) {
+            while (R[rlen - 1] != 0u && minus < CORR_MAX) {
                 ++minus;
                 lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
                 lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
@@ -296,7 +300,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         if (minus == 1) count(CNT_DELTA_NEG);
         if (minus > 1) count(CNT_DELTA_NEG_MULTI);
         int plus = 0;
-        for (int step = 0; step < 8; ++step) {             // r >= v: delta = +1 (once by Theorem 2 as printed)
+        for (int step = 0; step < CORR_MAX; ++step) {      // r >= v: delta = +1 (once by Theorem 2 as printed)
             const uint32_t borrow =
                 lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
             if (borrow) break;
@@ -306,7 +310,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
         if (plus == 1) count(CNT_DELTA_POS);
         if (plus > 1) count(CNT_DELTA_MULTI);
-        if (plus >= 8 || minus >= 8) count(CNT_DELTA_OUT_OF_RANGE);
+        if (plus >= CORR_MAX || minus >= CORR_MAX) count(CNT_DELTA_OUT_OF_RANGE);
         PHASE(6);
 
         // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
