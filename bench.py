@@ -39,7 +39,7 @@ IMAD_PER_CLK_PER_SM = 64
 FLUSH_BYTES = 256 << 20   # > 126 MB of L2
 
 # DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_final.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 15374336 + 1443584, 3: 38150144 + 15338752, 4: 37935872 + 14671872}
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 15372288 + 1470464, 3: 38213888 + 26464512, 4: 38073088 + 25319168}
 
 
 def parse_args():
