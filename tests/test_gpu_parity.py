@@ -198,6 +198,20 @@ def test_div_directed(M, n, count, variant):
         assert cnt["delta_neg_multi"] == 0 and cnt["clipped_steps"] == 0
 
 
+@pytest.mark.parametrize("M,n,count", [(1024, 512, 4096), (2048, 1024, 4096), (2048, 2048, 2048), (4096, 2048, 2048),
+                                       (8192, 4096, 512)])
+def test_div_directed_large_sets(M, n, count):
+    """The directed set at the size SURVEY 8(d) asks for (thousands per size) on the default variant: the clipped
+    products, the "+1" Refine loop and the tensor-core range products must leave every quotient within reach of
+    the correction loops."""
+    binding.debug_counters(reset=True)
+    u, v = inputs.directed(M, n, count=count, seed=inputs.SEED + 17)
+    check_div(u, v, "directed (large set) M=%d n=%d" % (M, n))
+    cnt = binding.debug_counters(reset=True)
+    print("counters", cnt)
+    assert cnt["delta_out_of_range"] == 0 and cnt["mma_wait_failures"] == 0
+
+
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_directed_reaches_corner_paths(variant):
     """The directed set must actually drive the rare branches: delta = -1, delta = +1,
