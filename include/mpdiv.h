@@ -115,6 +115,23 @@ int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_lim
                    int batch, int variant, mpdiv_stream_t stream);
 
 /*
+ * The linear-cost building blocks of the method on their own (PAPER.md 3.2-3.3), exported so that they can
+ * be unit-tested: each is the block-level map-scan-map the division uses internally.
+ *   a : batch x a_limbs, b : batch x b_limbs (device, read);  out : batch x out_limbs, flag : batch words
+ *   (device, written).  shift counts whole limbs; shift_n(x) = floor(x * B^n) (Definition 1).
+ *   MPLINOP_ADD    out = (a + shift_n(b)) mod B^out_limbs,  flag = carry out
+ *   MPLINOP_SUB    out = (a - shift_n(b)) mod B^out_limbs,  flag = borrow out = (a < shift_n(b)) when both fit
+ *                  in out_limbs: subtraction with the borrow scan and the less-than test (:331-335, :343-440)
+ *   MPLINOP_NEG    out = B^shift - a (a < B^shift <= B^out_limbs), the B^L - P of PowDiff (:117, :329); flag = carry
+ *   MPLINOP_SHIFT  out = shift_n(a) truncated to out_limbs (n = shift, either sign)    (:204)
+ *   MPLINOP_PREC   flag = prec(a) = number of significant limbs (:135);  out = a
+ *   MPLINOP_ANY    flag = 1 when a limb of a at index >= shift is non-zero (the comparison with B^h, :329); out = a
+ */
+enum { MPLINOP_ADD = 0, MPLINOP_SUB = 1, MPLINOP_NEG = 2, MPLINOP_SHIFT = 3, MPLINOP_PREC = 4, MPLINOP_ANY = 5 };
+int mplinop_batch(int op, const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, int shift,
+                  uint32_t *out, int out_limbs, uint32_t *flag, int batch, mpdiv_stream_t stream);
+
+/*
  * Host-buffer form of mpdiv_batch for end-to-end use: u, v, q, r are HOST pointers (pinned memory
  * recommended; pageable memory works but serialises the copies); `workspace` is a caller-owned DEVICE
  * buffer of at least mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch) bytes.  The batch is cut into

@@ -21,6 +21,7 @@ OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
 VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
 VARIANT_DEFAULT = VARIANT_CLIPPED
 ENGINE_IMAD, ENGINE_TENSOR = 0, 1
+LINOP_ADD, LINOP_SUB, LINOP_NEG, LINOP_SHIFT, LINOP_PREC, LINOP_ANY = range(6)
 MAX_LIMBS = 8192
 
 
@@ -43,6 +44,7 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
         L.mpdiv_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, i, _VOIDP]
         L.shinv_batch_ex.argtypes = [_VOIDP, i, i, _VOIDP, i, i, i, _VOIDP]
+        L.mplinop_batch.argtypes = [i, _VOIDP, i, _VOIDP, i, i, _VOIDP, i, _VOIDP, i, _VOIDP]
         L.mpmul_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, i, _VOIDP]
         L.mpmul_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, _VOIDP]
         L.shinv_batch.argtypes = [_VOIDP, i, i, _VOIDP, i, i, _VOIDP]
@@ -55,14 +57,14 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_version.restype = ctypes.c_char_p
         L.mpdiv_strerror.argtypes = [i]
         L.mpdiv_strerror.restype = ctypes.c_char_p
-        for name in ("mpdiv_batch", "mpdiv_batch_ex", "shinv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "mpdiv_batch_host",
+        for name in ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "shinv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "mpdiv_batch_host",
                      "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_debug_counters"):
             getattr(L, name).restype = i
         _LIB = L
     return _LIB
 
 
-EXPORTS = ("mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
+EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
            "mpdiv_debug_counters", "mpdiv_version", "mpdiv_strerror")
 
@@ -139,6 +141,18 @@ def mpmul_batch(a: torch.Tensor, b: torch.Tensor, c_limbs: int, c: torch.Tensor 
         _raise(lib().mpmul_batch_ex(a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], c.data_ptr(), c_limbs, batch,
                                     int(engine), _stream_ptr(stream)), "mpmul_batch_ex")
     return c
+
+
+def mplinop_batch(op: int, a: torch.Tensor, b: torch.Tensor, shift: int, out_limbs: int, stream=None):
+    """One linear building block per row (include/mpdiv.h); returns (out, flag)."""
+    _check_dev(a, "a")
+    _check_dev(b, "b")
+    batch = a.shape[0]
+    out = torch.empty((batch, out_limbs), dtype=a.dtype, device=a.device)
+    flag = torch.empty((batch,), dtype=torch.int32, device=a.device)
+    _raise(lib().mplinop_batch(int(op), a.data_ptr(), a.shape[1], b.data_ptr(), b.shape[1], int(shift), out.data_ptr(),
+                               out_limbs, flag.data_ptr(), batch, _stream_ptr(stream)), "mplinop_batch")
+    return out, flag
 
 
 def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = None, stream=None,

@@ -326,6 +326,52 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     }
 }
 
+
+// ---------------------------------------------------------------------------------------
+// mplinop_batch: the linear-cost building blocks of mp_block.cuh on their own (unit tests)
+// ---------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(T)
+mplinop_kernel(int op, const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b, int b_limbs, int shift,
+               limb *__restrict__ out, int out_limbs, uint32_t *__restrict__ flag, int batch)
+{
+    extern __shared__ __align__(1024) uint32_t smem[];
+    const int ap = round_up(a_limbs, TILE) + TILE, bp = round_up(b_limbs, TILE) + TILE, op_ = round_up(out_limbs, TILE);
+    limb *A = smem, *Bs = A + ap, *O = Bs + bp;
+    Blk blk{reinterpret_cast<BlkScratch *>(O + op_ + TILE), 0u, 0u};
+    for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
+        load_number<T>(A, a + (size_t)inst * a_limbs, a_limbs, ap);
+        load_number<T>(Bs, b + (size_t)inst * b_limbs, b_limbs, bp);
+        __syncthreads();
+        uint32_t f = 0;
+        switch (op) {
+            case MPLINOP_ADD:      // out = (a + shift_n(b)) mod B^out_limbs, flag = carry out
+                f = lin_addsub<T, false>(O, op_, LimbView{A, a_limbs, 0}, LimbView{Bs, b_limbs, -shift}, 0u, blk);
+                break;
+            case MPLINOP_SUB:      // out = (a - shift_n(b)) mod B^out_limbs, flag = borrow = (a < shift_n(b))  (:343-440, :331-335)
+                f = lin_addsub<T, true>(O, op_, LimbView{A, a_limbs, 0}, LimbView{Bs, b_limbs, -shift}, 0u, blk);
+                break;
+            case MPLINOP_NEG:      // out = B^shift - a for a < B^shift (the B^L - P of PowDiff)
+                f = lin_addsub<T, false>(O, op_, NotView{A, shift, a_limbs}, ZeroView{}, 1u, blk);
+                break;
+            case MPLINOP_SHIFT:    // out = shift_n(a), whole limbs, n = shift of either sign   (Definition 1)
+                lin_copy<T>(O, op_, A, a_limbs, -shift);
+                break;
+            case MPLINOP_PREC:     // flag = prec(a); out = a
+                f = (uint32_t)prec_of<T>(A, a_limbs, blk);
+                lin_copy<T>(O, op_, A, a_limbs, 0);
+                break;
+            default:               // MPLINOP_ANY: flag = any limb of a[shift, a_limbs) non-zero; out = a
+                f = any_nonzero<T>(A, shift, a_limbs) ? 1u : 0u;
+                lin_copy<T>(O, op_, A, a_limbs, 0);
+                break;
+        }
+        store_number<T>(out + (size_t)inst * out_limbs, O, out_limbs, min(op_, out_limbs));
+        if (threadIdx.x == 0) flag[inst] = f;
+        __syncthreads();
+    }
+}
+
 // ---------------------------------------------------------------------------------------
 // host side of mpdiv_batch / shinv_batch / host-buffer form / counters
 // ---------------------------------------------------------------------------------------
@@ -448,6 +494,35 @@ int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_lim
         case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st, clip);
         default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st, clip);
     }
+}
+
+
+int mplinop_batch(int op, const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs, int shift, uint32_t *out,
+                  int out_limbs, uint32_t *flag, int batch, mpdiv_stream_t stream)
+{
+    if (!a || !b || !out || !flag || a_limbs <= 0 || b_limbs <= 0 || out_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
+    if (op < MPLINOP_ADD || op > MPLINOP_ANY) return MPDIV_ERR_BAD_ARG;
+    if ((a_limbs | b_limbs | out_limbs) & 3) return MPDIV_ERR_BAD_ARG;
+    if (!aligned16(a) || !aligned16(b) || !aligned16(out)) return MPDIV_ERR_BAD_ARG;
+    if (a_limbs > MPDIV_MAX_LIMBS || b_limbs > MPDIV_MAX_LIMBS || out_limbs > 2 * MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (shift < -2 * MPDIV_MAX_LIMBS || shift > 2 * MPDIV_MAX_LIMBS) return MPDIV_ERR_BAD_ARG;
+    if ((op == MPLINOP_NEG && (shift < 0 || shift > out_limbs)) || (op == MPLINOP_ANY && shift < 0)) return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const size_t words = (size_t)round_up(a_limbs, TILE) + round_up(b_limbs, TILE) + round_up(out_limbs, TILE) + 3 * TILE +
+                         sizeof(BlkScratch) / 4;
+    const size_t bytes = words * 4;
+    const int big = out_limbs > a_limbs ? out_limbs : a_limbs;
+    if (big <= 1024) {
+        int rc = set_smem(mplinop_kernel<128>, bytes);
+        if (rc != MPDIV_OK) return rc;
+        mplinop_kernel<128><<<batch, 128, bytes, st>>>(op, a, a_limbs, b, b_limbs, shift, out, out_limbs, flag, batch);
+    } else {
+        int rc = set_smem(mplinop_kernel<512>, bytes);
+        if (rc != MPDIV_OK) return rc;
+        mplinop_kernel<512><<<batch, 512, bytes, st>>>(op, a, a_limbs, b, b_limbs, shift, out, out_limbs, flag, batch);
+    }
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
 size_t mpdiv_host_workspace_bytes(int u_limbs, int v_limbs, int batch)
