@@ -20,7 +20,7 @@ def test_library_builds_and_exports_every_declared_symbol():
     lib = ctypes.CDLL(path)
     header = open(os.path.join(ROOT, "include", "mpdiv.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b((?:mpdiv|mpmul|shinv)_\w+)\s*\(", header))
+    declared = set(re.findall(r"\b((?:mpdiv|mpmul|mplinop|shinv)_\w+)\s*\(", header))
     assert {"mpdiv_batch", "mpmul_batch", "shinv_batch"} <= declared
     for name in declared:
         assert hasattr(lib, name), "libmpdiv.so does not export %s" % name
