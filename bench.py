@@ -420,6 +420,15 @@ def run_ours(args):
     if not args.brief:
         out["per_config"] = per_config_table(binding, flush, peak_products)
         out["paper_shape"] = paper_shape_table(binding, flush)
+        # config 1 has 32 instances (latency bound on 148 SMs); the same shape with 32 x 148 instances gives the
+        # THROUGHPUT point of the metric at 2^15 bits
+        u15, v15 = inputs.uniform_operands(32 * 148, 1024, 512, config=11)
+        d15u, d15v = to_dev(u15), to_dev(v15)
+        q15, r15 = torch.empty_like(d15u), torch.empty_like(d15v)
+        t15 = float(np.median(time_steps(lambda: binding.mpdiv_batch(d15u, d15v, q15, r15), 25, 3, flush)))
+        out["throughput_2^15_bits"] = {"batch": 32 * 148, "u_limbs": 1024, "v_limbs": 512, "div_ms": t15,
+                                       "div_per_s": 32 * 148 / (t15 * 1e-3),
+                                       "roofline_frac": 32 * 148 / (t15 * 1e-3) * W_LIMB_PRODUCTS[1024] / peak_products}
         out["cpu_baseline"] = cpu_baseline(cfg)
         out["paper_context"] = "A100, 64-bit digits (PAPER.md:481-484): div/mul 6.77x/6.66x/6.94x/9.73x at 2^18..2^15 bits; model 5-7"
     print(json.dumps(out))
