@@ -18,8 +18,10 @@
 //     from registers into TENSOR MEMORY (`tcgen05.st`, lane = row, 32 columns = 128 bytes of K) and the
 //     MMA takes its A operand from there (`tcgen05.mma [d], [a_tmem], b_desc`): the tile never touches
 //     shared memory, whose bandwidth was the limit of a first version that staged A tiles in a 16 KB ring
-//     (about 840 cycles per step against 530 for the four MMAs).  Stages of 32 TMEM columns are handed to
-//     the single MMA-issuing thread through mbarriers and freed by `tcgen05.commit`.
+//     (about 840 cycles per step).  With A in tensor memory a step takes 690 cycles, which is the rate of
+//     the TS-form MMA itself (172 cycles per instruction against 132 with A in shared memory, measured with
+//     the waits removed).  Stages of 32 TMEM columns are handed to the single MMA-issuing thread through
+//     mbarriers and freed by `tcgen05.commit`.
 //   * Epilogue: `tcgen05.ld` (lane = i, column = d), four adjacent lanes form one limb's 64-bit column
 //     sum, low words go to P, high words to HI one limb up, and one block-wide carry-propagating add
 //     (mp_block.cuh) finishes.
