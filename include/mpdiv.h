@@ -171,9 +171,22 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
  *   out[9] instances needing more than one -1 step      out[10] instances whose correction loops hit
  *          their bound of 64 (result not exact; expected 0)      out[11] Newton steps that ran clipped
  *   out[12] range products that ran on the tensor core (mp_mma.cuh)      out[13] bit mask of tensor-core
- *          pipeline waits that gave up (expected 0)      out[14..15] reserved (0)
+ *          pipeline waits that gave up (expected 0)
+ *   out[14] add-back steps of the seed's long division (Knuth D6)      out[15] Shinv calls that started
+ *          Refine from the 17-digit seed (mpdiv_seed_batch)
  */
 int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream);
+
+/*
+ * The seed of Refine (clipped variant, csrc/mp_div.cuh warp_seed): for each divisor v >= B,
+ *      w[i] = floor(B^38 / D),  D = floor(v * B^19 / B^k),  k = prec(v) - 1
+ * i.e. the exact quotient of B^38 by the top 20 limbs of v, which stands in for the first four Refine
+ * iterations (Alg. 1 lines 19-25, l = 2 -> 17) when h - k >= 17.  One warp per divisor,
+ * schoolbook long division with one limb per lane.  Exposed so that the tests can pin the routine on its own.
+ *   v   device, batch x v_limbs limbs, little endian          w   device, batch x 24 limbs (20 significant)
+ * A divisor with fewer than two significant limbs yields 24 zero limbs.
+ */
+int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpdiv_stream_t stream);
 
 /* "mpdiv <version> sm_100a ..." */
 const char *mpdiv_version(void);

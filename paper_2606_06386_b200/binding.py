@@ -54,6 +54,7 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_imad_probe_threads.argtypes = []
         L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
         L.mpdiv_debug_counters.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), i, _VOIDP]
+        L.mpdiv_seed_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP]
         L.mpdiv_version.restype = ctypes.c_char_p
         L.mpdiv_strerror.argtypes = [i]
         L.mpdiv_strerror.restype = ctypes.c_char_p
@@ -66,7 +67,7 @@ def lib() -> ctypes.CDLL:
 
 EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
-           "mpdiv_debug_counters", "mpdiv_version", "mpdiv_strerror")
+           "mpdiv_debug_counters", "mpdiv_seed_batch", "mpdiv_version", "mpdiv_strerror")
 
 
 def version() -> str:
@@ -172,6 +173,22 @@ def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = 
     return w
 
 
+SEED_LIMBS = 24     # limbs per row of mpdiv_seed_batch (20 significant)
+
+
+def seed_batch(v: torch.Tensor, w: torch.Tensor | None = None, stream=None):
+    """w = floor(B^38 / (top 20 limbs of v)) per row: the 17-digit seed of Refine (include/mpdiv.h)."""
+    _check_dev(v, "v")
+    if w is None:
+        w = torch.empty((v.shape[0], SEED_LIMBS), dtype=v.dtype, device=v.device)
+    _check_dev(w, "w")
+    if w.shape != (v.shape[0], SEED_LIMBS):
+        raise ValueError("w must be batch x %d" % SEED_LIMBS)
+    _raise(lib().mpdiv_seed_batch(v.data_ptr(), v.shape[1], w.data_ptr(), v.shape[0], _stream_ptr(stream)),
+           "mpdiv_seed_batch")
+    return w
+
+
 def host_workspace_bytes(u_limbs: int, v_limbs: int, batch: int) -> int:
     return int(lib().mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch))
 
@@ -208,7 +225,7 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
                  "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "mma_products", "mma_wait_failures",
-                 "rsv14", "rsv15")
+                 "seed_addbacks", "seeds")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:

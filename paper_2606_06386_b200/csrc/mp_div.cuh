@@ -34,7 +34,7 @@ namespace mpd {
 __device__ unsigned long long g_counters[16];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
        CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
-       CNT_MMA_PRODUCTS };
+       CNT_MMA_PRODUCTS, CNT_MMA_WAIT_FAILURES /* filled by the host from mp_mma.cuh */, CNT_SEED_ADDBACK, CNT_SEEDS };
 
 // Phase timing for tuning builds only (-DMPDIV_PHASE_TIMING): thread 0 of block 0 accumulates the cycles
 // between consecutive PHASE() marks.  Compiles to nothing in the product build.
@@ -228,11 +228,117 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     PHASE(32 + (it & 15));
 }
 
+// ---------------------------------------------------------------------------------------
+// Seed of Refine with 17 correct digits, computed by one warp (clipped variant only).
+//
+// Refine's iterate with l correct digits is w ~ B^(k+l+g) / v (PAPER.md:92 l.15-25).  The first four
+// iterations (l = 2, 3, 5, 9 -> 17) multiply numbers of 4 to 40 limbs and cost ~10 000 cycles each in
+// block-wide barriers and scans; they are replaced by the exact quotient
+//      w = floor(B^38 / D),   D = floor(v / B^(k-19))   (the top 20 limbs of v; v * B^(19-k) when k < 19),
+// which satisfies  B^(k+19)/v - 1 < w <= B^(k+19)/v + 1  because D <= v/B^(k-19) < D + 1 and D >= B^19:
+// a better iterate than the one Refine would hold at l = 17 (whose error is several units of a guard limb).
+// The quotient comes from schoolbook long division (Knuth, TAOCP vol. 2, 4.3.1 Algorithm D) with one limb
+// per lane: lane j holds limb j of the normalised divisor and of the 21-limb remainder window; a quotient
+// digit is a 2-by-1 division by the top divisor limb through its precomputed reciprocal (Moeller and
+// Granlund, "Improved division by invariant integers", Alg. 4), Knuth's two-digit test, a multiply-subtract
+// whose carries and borrows are resolved by two ballots and an integer add, and a rare add-back.
+// ---------------------------------------------------------------------------------------
+constexpr int SEED_L = 17;                 // correct digits of the seed
+constexpr int SEED_ITERS = 4;              // Refine iterations it replaces (l = 2 -> 3 -> 5 -> 9 -> 17)
+constexpr int SEED_LIMBS = SEED_L + 3;     // limbs of D and of the quotient (l + g + 1)
+
+// carries into each lane from generate / propagate masks: bit j of the result = carry into lane j
+__device__ __forceinline__ uint32_t lane_carries(uint32_t G, uint32_t P)
+{
+    return ((G | P) + G) ^ P;              // G and P are disjoint
+}
+
+// Runs on one full warp.  W receives SEED_LIMBS limbs and zeros up to 24 (the wlen of iteration 4).
+__device__ __forceinline__ void warp_seed(const limb *V, int k, limb *W)
+{
+    constexpr uint32_t FULL = 0xffffffffu;
+    constexpr int ND = SEED_LIMBS;
+    const int lane = threadIdx.x & 31;
+    const int idx = k - (ND - 1) + lane;
+    const uint32_t dj = (lane < ND && idx >= 0) ? V[idx] : 0u;
+    // D1: normalise so that the top limb has its high bit set (the dividend B^38 shifts with it)
+    const int sh = __clz(__shfl_sync(FULL, dj, ND - 1));
+    uint32_t dl = __shfl_up_sync(FULL, dj, 1);
+    if (lane == 0) dl = 0u;
+    const uint32_t d = (lane < ND) ? __funnelshift_l(dl, dj, sh) : 0u;
+    const uint32_t d1 = __shfl_sync(FULL, d, ND - 1), d0 = __shfl_sync(FULL, d, ND - 2);
+    const uint32_t dinv = (uint32_t)(0xffffffffffffffffull / d1);      // floor((B^2 - 1) / d1) - B
+    // remainder window: lane j holds limb i + j of the running remainder at quotient digit i; digit ND-1 first,
+    // where the only non-zero limb of B^38 << sh is limb 38 = lane 19
+    uint32_t r = (lane == ND - 1) ? (1u << sh) : 0u;
+    uint32_t qd = 0u;
+    uint32_t addbacks = 0u;
+#pragma unroll 1
+    for (int i = ND - 1; i >= 0; --i) {
+        const uint32_t r2 = __shfl_sync(FULL, r, ND), r1 = __shfl_sync(FULL, r, ND - 1), r0 = __shfl_sync(FULL, r, ND - 2);
+        // D3: qhat = min(floor((r2 B + r1) / d1), B - 1), rhat the remainder; then the two-digit test
+        uint32_t qh, rh;
+        bool test = true;
+        if (r2 >= d1) {                                       // r2 = d1 (r2 > d1 cannot happen)
+            qh = 0xffffffffu;
+            rh = r1 + d1;
+            test = rh >= d1;                                  // no overflow: rhat < B
+        } else {
+            const uint64_t pq = (uint64_t)dinv * r2 + (((uint64_t)r2 << 32) | r1);
+            uint32_t q1 = (uint32_t)(pq >> 32) + 1u;
+            const uint32_t q0 = (uint32_t)pq;
+            rh = r1 - q1 * d1;
+            if (rh > q0) { q1 -= 1u; rh += d1; }
+            if (rh >= d1) { q1 += 1u; rh -= d1; }
+            qh = q1;
+        }
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            if (test && (uint64_t)qh * d0 > (((uint64_t)rh << 32) | r0)) {
+                qh -= 1u;
+                const uint32_t nr = rh + d1;
+                test = nr >= rh;                              // stop once rhat >= B
+                rh = nr;
+            }
+        }
+        // D4: r -= qhat * D over the 21 lanes
+        const uint64_t p = (uint64_t)qh * d;
+        uint32_t hp = __shfl_up_sync(FULL, (uint32_t)(p >> 32), 1);
+        if (lane == 0) hp = 0u;
+        uint32_t t = (uint32_t)p + hp;
+        uint32_t G = __ballot_sync(FULL, t < hp), P = __ballot_sync(FULL, t == 0xffffffffu);
+        t += (lane_carries(G, P) >> lane) & 1u;
+        uint32_t s = r - t;
+        G = __ballot_sync(FULL, r < t);
+        P = __ballot_sync(FULL, r == t);
+        uint32_t bw = lane_carries(G, P);
+        s -= (bw >> lane) & 1u;
+        // D5/D6: negative remainder (borrow out of lane ND): add the divisor back (probability ~2/B per digit)
+        bool neg = ((bw >> (ND + 1)) & 1u) != 0u;
+        while (neg) {
+            qh -= 1u;
+            addbacks += 1u;
+            const uint32_t s2 = s + d;
+            G = __ballot_sync(FULL, s2 < s);
+            P = __ballot_sync(FULL, s2 == 0xffffffffu);
+            const uint32_t cw = lane_carries(G, P);
+            s = s2 + ((cw >> lane) & 1u);
+            neg = ((cw >> (ND + 1)) & 1u) == 0u;              // the carry out of lane ND cancels the borrow
+        }
+        if (lane == i) qd = qh;
+        // D7: next digit: the window moves one limb down (the dividend's lower limbs are all zero)
+        r = __shfl_up_sync(FULL, s, 1);
+        if (lane == 0) r = 0u;
+    }
+    if (lane < 24) W[lane] = (lane < ND) ? qd : 0u;
+    if (lane == 0 && addbacks) atomicAdd(&g_counters[CNT_SEED_ADDBACK], (unsigned long long)addbacks);
+}
+
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
-                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0)
+                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
     const MulScratch &ms = bufs.ms;
@@ -269,7 +375,18 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     const int iters = ((H - 1 > 1) ? (32 - __clz(H - 2)) : 0) + (clip ? 1 : 2);
     limb *Wc = ((iters + 1) & 1) ? WB : WA;                    // so that write number iters+1 hits WA
     limb *Wn = (Wc == WA) ? WB : WA;
-    if (threadIdx.x == 0) {
+    int l = 2;
+    int wlen = TILE;                                           // valid (zero padded) words of Wc
+    int it0 = 0;
+    if (clip && seed && H >= SEED_L) {
+        // the first four iterations would all double l (m = l up to l = 9 needs H + 1 - 9 >= 9): start from the
+        // 17-digit seed instead; Wc is the buffer iteration 4 reads (an even number of swaps away)
+        if (threadIdx.x < 32) warp_seed(V, k, Wc);
+        count(CNT_SEEDS);
+        l = SEED_L;
+        wlen = 24;
+        it0 = SEED_ITERS;
+    } else if (threadIdx.x == 0) {
         const unsigned long long V2 = ((unsigned long long)V[k] << 32) | V[k - 1];
         const unsigned __int128 w0 = (((unsigned __int128)1) << 96) / V2;
         Wc[0] = 0u; Wc[1] = 0u;                                // shift_g(w), g = 2 (Alg. 1 line 17)
@@ -277,8 +394,6 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
         Wc[5] = 0u; Wc[6] = 0u; Wc[7] = 0u;
     }
     __syncthreads();
-    int l = 2;
-    int wlen = TILE;                                           // valid (zero padded) words of Wc
 
     // ---- Refine (Alg. 1 lines 15-28) ------------------------------------------------------------
     PHASE(0);
@@ -286,7 +401,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     // (narrow_l = 33 when the grid has more blocks than SMs: a lone block per SM is latency bound and keeps all
     // its threads; 0 disables)
     bool narrow_open = false;
-    for (int it = 0; it < iters; ++it) {
+    for (int it = it0; it < iters; ++it) {
         const int m = min(H + 1 - l, l);
         const int nlen = round_up(l + m + g + 2, TILE);
         if (T > 32 && l <= narrow_l && it + 2 < iters) {

@@ -81,6 +81,26 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
 }
 
 // ---------------------------------------------------------------------------------------
+// mpdiv_seed_batch kernel: the 17-digit seed of Refine on its own (one warp per divisor, v read from HBM)
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+seed_kernel(const limb *__restrict__ v, int v_limbs, limb *__restrict__ w, int batch)
+{
+    const int inst = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (inst >= batch) return;
+    const limb *V = v + (size_t)inst * v_limbs;
+    int top = -1;                                             // index of the top non-zero limb
+    for (int i0 = 0; i0 < v_limbs; i0 += 32) {
+        const int i = i0 + lane;
+        const uint32_t nz = __ballot_sync(0xffffffffu, i < v_limbs && V[i] != 0u);
+        if (nz) top = i0 + 31 - __clz(nz);
+    }
+    limb *W = w + (size_t)inst * 24;
+    if (top < 1) { if (lane < 24) W[lane] = 0u; return; }
+    warp_seed(V, top, W);
+}
+
+// ---------------------------------------------------------------------------------------
 // shinv_batch kernel
 // ---------------------------------------------------------------------------------------
 template <int T>
@@ -111,9 +131,9 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
             count(CNT_ONE_LIMB);
             if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }   // v*B at the (aligned) base V
             __syncthreads();
-            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0, nullptr, narrow_l);
+            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0, nullptr, narrow_l & 255, !(narrow_l & 256));
         } else {
-            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0, nullptr, narrow_l);
+            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0, nullptr, narrow_l & 255, !(narrow_l & 256));
         }
         store_number<T>(wout, bufs.WA, w_limbs, round_up(nw, TILE));
         __syncthreads();
@@ -207,7 +227,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
         PHASE(1);
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l);
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256));
         const int psh = top_prec(WA, nw);
         PHASE(2);
 
@@ -384,7 +404,8 @@ struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; 
 
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
-int narrow_for(int batch) { return batch > g_sm_count ? 33 : 0; }
+// low byte: l up to which Refine runs on warp 0 alone; bit 8: MPDIV_NO_SEED (tuning: start Refine at l = 2)
+int narrow_for(int batch) { return (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0); }
 
 template <int T, bool LAT>
 int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
@@ -618,6 +639,14 @@ int mpdiv_debug_phases(unsigned long long out[64], int reset)
     return MPDIV_OK;
 }
 #endif
+
+int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpdiv_stream_t stream)
+{
+    if (!v || !w || v_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    seed_kernel<<<(batch + 3) / 4, 128, 0, reinterpret_cast<cudaStream_t>(stream)>>>(v, v_limbs, w, batch);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
 
 int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream)
 {
