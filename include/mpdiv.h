@@ -135,9 +135,10 @@ int mplinop_batch(int op, const uint32_t *a, int a_limbs, const uint32_t *b, int
  * Host-buffer form of mpdiv_batch for end-to-end use: u, v, q, r are HOST pointers (pinned memory
  * recommended; pageable memory works but serialises the copies); `workspace` is a caller-owned DEVICE
  * buffer of at least mpdiv_host_workspace_bytes(u_limbs, v_limbs, batch) bytes.  The batch is cut into
- * chunks of about one wave of the kernel; the H2D copy of chunk i+1 and the D2H copy of chunk i-1
- * overlap the division of chunk i on two library-owned helper streams (created on first use, never
- * destroyed).  Everything is ordered after the work already enqueued on `stream`, and `stream`
+ * up to 16 chunks of about one division per SM; the H2D copy of chunk i+1 and the D2H copy of chunk i-1
+ * overlap the division of chunk i, and the chunk kernels rotate over four streams so that consecutive
+ * chunks share the SMs as the blocks of one launch would (six library-owned helper streams, created on
+ * first use, never destroyed).  Everything is ordered after the work already enqueued on `stream`, and `stream`
  * completes only after the last D2H copy: the caller synchronises `stream` and reads q, r.
  * Reuse of the same events makes concurrent calls from several host threads unsupported.
  */

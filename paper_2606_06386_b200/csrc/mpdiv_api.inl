@@ -152,8 +152,11 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // bound only has to keep |delta| * v below B^(k+2), the range of the remainder arithmetic.
 constexpr int CORR_MAX = 64;
 
+#ifndef MPDIV_B128
+#define MPDIV_B128 4      // resident 128-thread blocks per SM the register budget is set for
+#endif
 template <int T, bool LAT>
-__global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
+__global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : (T == 128 ? MPDIV_B128 : 512 / T))
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l)
 {
@@ -409,37 +412,26 @@ int narrow_for(int batch) { return (batch > g_sm_count ? 33 : 0) | (getenv("MPDI
 
 template <int T, bool LAT>
 int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-                 cudaStream_t st, int clip)
+                 cudaStream_t st, int clip, int sched)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(batch));
+    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched));
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
+// sched = the number of divisions that share the GPU with this launch (the batch itself, or the whole batch
+// when the host path launches it chunk by chunk on several streams): it picks the kernel flavour.
 template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-               cudaStream_t st, int clip)
+               cudaStream_t st, int clip, int sched)
 {
     // a batch of at most two blocks per SM is latency bound: give its threads all the registers they want
-    if (T <= 256 && batch <= 2 * g_sm_count) return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-    return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-}
-
-// divisions one wave of the division kernel holds on the whole GPU (blocks per SM x SMs)
-template <int T>
-int div_wave(int u_limbs, int v_limbs, int clip)
-{
-    DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    if (MmaEnabled<T>::value && clip && !getenv("MPDIV_NO_MMA")) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
-    const size_t bytes = (size_t)L.total_words * 4;
-    if (set_smem(mpdiv_kernel<T, false>, bytes) != MPDIV_OK) return 0;
-    int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, mpdiv_kernel<T, false>, T, bytes) != cudaSuccess) return 0;
-    return nb * g_sm_count;
+    if (T <= 256 && sched <= 2 * g_sm_count) return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+    return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
 }
 
 template <int T>
@@ -473,6 +465,17 @@ int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, 
     return mpdiv_batch_ex(u, u_limbs, v, v_limbs, q, r, batch, MPDIV_VARIANT_DEFAULT, stream);
 }
 
+static int div_dispatch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
+                        int batch, int clip, cudaStream_t st, int sched)
+{
+    switch (threads_for(u_limbs)) {
+        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+    }
+}
+
 int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
                    int batch, int variant, mpdiv_stream_t stream)
 {
@@ -482,13 +485,7 @@ int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limb
     if (rc != MPDIV_OK) return rc;
     if (!aligned16(u) || !aligned16(v) || !aligned16(q) || !aligned16(r)) return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
-    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    switch (threads_for(u_limbs)) {
-        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st, clip);
-    }
+    return div_dispatch(u, u_limbs, v, v_limbs, q, r, batch, clip, reinterpret_cast<cudaStream_t>(stream), batch);
 }
 
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch,
@@ -567,26 +564,24 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     uint32_t *dq = dv + (size_t)batch * v_limbs;
     uint32_t *dr = dq + (size_t)batch * u_limbs;
 
-    // Chunks of about one wave of the kernel: the upload of chunk i+1 and the download of chunk i-1
-    // overlap the division of chunk i (two helper streams, created once; events order the three).
-    int wave = 0;
-    switch (threads_for(u_limbs)) {
-        case 64: wave = div_wave<64>(u_limbs, v_limbs, 1); break;
-        case 128: wave = div_wave<128>(u_limbs, v_limbs, 1); break;
-        case 256: wave = div_wave<256>(u_limbs, v_limbs, 1); break;
-        default: wave = div_wave<512>(u_limbs, v_limbs, 1); break;
-    }
-    if (wave <= 0) return MPDIV_ERR_UNSUPPORTED;
-    constexpr int MAXC = 8;
-    int chunk = wave;
-    if ((batch + chunk - 1) / chunk > MAXC) chunk = ((batch + MAXC - 1) / MAXC + wave - 1) / wave * wave;
-    const int nchunks = (batch + chunk - 1) / chunk;
+    // Chunks of one division per SM (at most MAXC of them).  The upload of chunk i+1 and the download of chunk
+    // i-1 overlap the division of chunk i, and the chunk kernels go round NK streams so that the blocks of
+    // consecutive chunks share the SMs like the blocks of one launch would (a chunk alone would leave each SM
+    // with a single block); the kernel flavour is the one the whole batch would get.
+    constexpr int MAXC = 16, NK = 4;
+    int nchunks = batch / g_sm_count;
+    if (nchunks < 1) nchunks = 1;
+    if (nchunks > MAXC) nchunks = MAXC;
+    const int chunk = (batch + nchunks - 1) / nchunks;
+    nchunks = (batch + chunk - 1) / chunk;
 
-    static cudaStream_t s_in = nullptr, s_out = nullptr;
+    static cudaStream_t s_in = nullptr, s_out = nullptr, s_k[NK];
     static cudaEvent_t ev_start = nullptr, ev_in[MAXC], ev_k[MAXC], ev_done = nullptr;
     if (!s_in) {
         if (cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
         if (cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
+        for (int i = 0; i < NK; i++)
+            if (cudaStreamCreateWithFlags(&s_k[i], cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
         if (cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
         if (cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
         for (int i = 0; i < MAXC; i++) {
@@ -597,23 +592,23 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
 #define MPDIV_CK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return MPDIV_ERR_CUDA; } } while (0)
     MPDIV_CK(cudaEventRecord(ev_start, st));                  // the helpers start after earlier work on `stream`
     MPDIV_CK(cudaStreamWaitEvent(s_in, ev_start, 0));
-    MPDIV_CK(cudaStreamWaitEvent(s_out, ev_start, 0));
     for (int c = 0; c < nchunks; c++) {
         const size_t lo = (size_t)c * chunk;
         const int cnt = (int)((size_t)batch - lo < (size_t)chunk ? (size_t)batch - lo : (size_t)chunk);
         const size_t uo = lo * u_limbs, vo = lo * v_limbs;
+        cudaStream_t sk = s_k[c % NK];
         MPDIV_CK(cudaMemcpyAsync(du + uo, u_host + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyHostToDevice, s_in));
         MPDIV_CK(cudaMemcpyAsync(dv + vo, v_host + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyHostToDevice, s_in));
         MPDIV_CK(cudaEventRecord(ev_in[c], s_in));
-        MPDIV_CK(cudaStreamWaitEvent(st, ev_in[c], 0));
-        rc = mpdiv_batch(du + uo, u_limbs, dv + vo, v_limbs, dq + uo, dr + vo, cnt, stream);
+        MPDIV_CK(cudaStreamWaitEvent(sk, ev_in[c], 0));       // ev_in follows ev_start on s_in
+        rc = div_dispatch(du + uo, u_limbs, dv + vo, v_limbs, dq + uo, dr + vo, cnt, 1, sk, batch);
         if (rc != MPDIV_OK) return rc;
-        MPDIV_CK(cudaEventRecord(ev_k[c], st));
+        MPDIV_CK(cudaEventRecord(ev_k[c], sk));
         MPDIV_CK(cudaStreamWaitEvent(s_out, ev_k[c], 0));
         MPDIV_CK(cudaMemcpyAsync(q_host + uo, dq + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyDeviceToHost, s_out));
         MPDIV_CK(cudaMemcpyAsync(r_host + vo, dr + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyDeviceToHost, s_out));
     }
-    MPDIV_CK(cudaEventRecord(ev_done, s_out));
+    MPDIV_CK(cudaEventRecord(ev_done, s_out));                // s_out has waited for every chunk kernel
     MPDIV_CK(cudaStreamWaitEvent(st, ev_done, 0));            // `stream` completes when the last download has
 #undef MPDIV_CK
     return MPDIV_OK;
