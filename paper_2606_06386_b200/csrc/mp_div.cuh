@@ -42,7 +42,7 @@ enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT
 __device__ unsigned long long g_op[16];
 #define OPDECL() long long tacc_[8] = {0,0,0,0,0,0,0,0}; long long tt_ = clock64()
 #define OPT(i) do { long long t__ = clock64(); tacc_[i] += t__ - tt_; tt_ = t__; } while (0)
-#define OPFLUSH() do { if (blockIdx.x == 0 && threadIdx.x == 0 && it < 6) for (int i_ = 0; i_ < 8; i_++) atomicAdd(&g_op[i_], (unsigned long long)tacc_[i_]); } while (0)
+#define OPFLUSH() do { if (blockIdx.x == 0 && threadIdx.x == 0 && it >= 4 && it < 8) for (int i_ = 0; i_ < 8; i_++) atomicAdd(&g_op[i_], (unsigned long long)tacc_[i_]); } while (0)
 __device__ unsigned long long g_phase[64];
 __device__ long long g_phase_t0;
 #define PHASE(i)                                                        \
@@ -141,6 +141,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     if (L >= hpp) {
         // no room to truncate: full product and a comparison with B^h''
         mul_full<TT>(Vp, pv, Wc, pw, P, ms, blk);
+        OPT(4);
         const int pl = round_up(pv, TILE) + round_up(pw, TILE);
         positive = !any_nonzero<TT>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
         if (positive) {
@@ -176,6 +177,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
                 c = TILE * Klo2;
                 mul_range<TT>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
             }
+            OPT(4);
             xl = L - c;
             positive = P[xl - 1] != 0u;
             for (int i = threadIdx.x; i < round_up(xl, TILE); i += TT)
@@ -214,6 +216,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
             tl = mul_range<TT>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
             off = dd - TILE * Klo1;
         }
+        OPT(5);
         if (positive) {
             lin_addsub<TT, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, 0u, blk);
         } else {

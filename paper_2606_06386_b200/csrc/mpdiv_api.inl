@@ -429,8 +429,10 @@ template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
                cudaStream_t st, int clip, int sched)
 {
-    // a batch of at most two blocks per SM is latency bound: give its threads all the registers they want
-    if (T <= 256 && sched <= 2 * g_sm_count) return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+    // a batch that fits the SMs at the latency kernel's occupancy (two blocks per SM up to 128 threads, one at
+    // 256) is latency bound: give its threads all the registers they want
+    if (T <= 256 && sched <= (T <= 128 ? 2 : 1) * g_sm_count)
+        return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
     return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
 }
 
