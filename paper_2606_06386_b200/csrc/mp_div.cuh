@@ -337,11 +337,47 @@ __device__ __forceinline__ void warp_seed(const limb *V, int k, limb *W)
     if (lane == 0 && addbacks) atomicAdd(&g_counters[CNT_SEED_ADDBACK], (unsigned long long)addbacks);
 }
 
+// Refine's trip count for H = max(h - k, 2) (PAPER.md:92 l.18-19; "+1" for the clipped variant, see shinv_block).
+__device__ __forceinline__ int refine_iters(int H, bool clip)
+{
+    return ((H - 1 > 1) ? (32 - __clz(H - 2)) : 0) + (clip ? 1 : 2);
+}
+
+// ---------------------------------------------------------------------------------------
+// Head of Refine (clipped variant, throughput batches).  The iterations up to l = HEAD_L handle operands of
+// at most ~270 limbs: a few thousand limb products each, but thousands of cycles of dependent latency.  When
+// the blocks of a batch run them inside the division kernel, all resident blocks of an SM sit in these phases
+// at the same time (same sizes, same schedule) and the multiplier pipe idles.  A batch therefore runs them in a
+// kernel of its own, one WARP per divisor and up to 16 divisors per SM, which leaves the seed and the iterate
+// after the head (at most WMID_STRIDE limbs) in a workspace row; the division kernel starts Refine from there.
+// Both kernels derive the split from H alone (head_plan), so no flag travels with the row.
+// ---------------------------------------------------------------------------------------
+constexpr int HEAD_L = 129;                // the head runs the iterations that start with l <= HEAD_L ...
+constexpr int WMID_STRIDE = 272;           // ... and leaves at most 2 HEAD_L + g + 2 limbs, rounded up to tiles
+struct HeadPlan { int it_end, l_end, wlen_end; };   // it_end = 0: no head (Refine starts in the division kernel)
+
+__device__ __forceinline__ HeadPlan head_plan(int H, int iters)
+{
+    HeadPlan p{0, 0, 0};
+    if (H < SEED_L) return p;
+    int l = SEED_L, it = SEED_ITERS, wlen = 24;
+    while (l <= HEAD_L && it + 2 < iters) {                   // the last two iterations stay with the block
+        const int m = min(H + 1 - l, l);
+        wlen = round_up(l + m + 2 + 2, TILE);
+        l += m - 1;
+        ++it;
+    }
+    if (it == SEED_ITERS) return p;
+    p.it_end = it; p.l_end = l; p.wlen_end = wlen;
+    return p;
+}
+
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
-                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true)
+                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true,
+                                           const limb *wmid = nullptr)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
     const MulScratch &ms = bufs.ms;
@@ -375,13 +411,21 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     // repairs its truncation errors, and whatever is left is absorbed by the bounded correction loops of Div
     // (lambda stayed in {-1,0,1} on 60 000 random and directed cases of the big-integer model; a plain
     // `while l < H`, i.e. "+0", is wrong).
-    const int iters = ((H - 1 > 1) ? (32 - __clz(H - 2)) : 0) + (clip ? 1 : 2);
+    const int iters = refine_iters(H, clip);
     limb *Wc = ((iters + 1) & 1) ? WB : WA;                    // so that write number iters+1 hits WA
     limb *Wn = (Wc == WA) ? WB : WA;
     int l = 2;
     int wlen = TILE;                                           // valid (zero padded) words of Wc
     int it0 = 0;
-    if (clip && seed && H >= SEED_L) {
+    const HeadPlan hp = (clip && wmid) ? head_plan(H, iters) : HeadPlan{0, 0, 0};
+    if (hp.it_end) {
+        // the head kernel left the iterate after it_end iterations in the workspace row
+        if (hp.it_end & 1) { limb *t = Wc; Wc = Wn; Wn = t; }
+        for (int i = threadIdx.x; i < hp.wlen_end; i += T) Wc[i] = __ldg(wmid + i);
+        l = hp.l_end;
+        wlen = hp.wlen_end;
+        it0 = hp.it_end;
+    } else if (clip && seed && H >= SEED_L) {
         // the first four iterations would all double l (m = l up to l = 9 needs H + 1 - 9 >= 9): start from the
         // 17-digit seed instead; Wc is the buffer iteration 4 reads (an even number of swaps away)
         if (threadIdx.x < 32) warp_seed(V, k, Wc);
@@ -428,6 +472,48 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     const int rlen = round_up(h - k + 2, TILE);
     lin_copy<T>(Wn, rlen, Wc, wlen, sh);                       // Wn == WA by construction
     return h - k + 1;
+}
+
+// One divisor's head on one warp (blockDim.x == 32): seed, then the iterations head_plan assigns to it; the
+// iterate goes to wrow (hp.wlen_end limbs).  smem: HEAD_SMEM_WORDS words, 16-byte aligned.  vg is the divisor's
+// row in global memory; only its top 2 HEAD_L + 4 limbs are read.
+constexpr int HEAD_V = 288, HEAD_W = 272, HEAD_X = 288, HEAD_P = 448, HEAD_OV = 64;
+constexpr int HEAD_SMEM_WORDS = HEAD_V + 2 * HEAD_W + HEAD_X + 2 * HEAD_P + 2 * HEAD_OV + (int)(sizeof(BlkScratch) / 4);
+
+__device__ __forceinline__ void shinv_head_warp(const limb *__restrict__ vg, int k, int h, uint32_t *smem,
+                                                limb *__restrict__ wrow)
+{
+    const int lane = threadIdx.x;
+    const int H = max(h - k, 2);
+    const HeadPlan hp = head_plan(H, refine_iters(H, true));
+    if (!hp.it_end) return;
+    limb *Vs = smem, *Wc = Vs + HEAD_V, *Wn = Wc + HEAD_W, *X = Wn + HEAD_W, *P = X + HEAD_X;
+    MulScratch ms;
+    ms.HI = P + HEAD_P;
+    ms.OV = ms.HI + HEAD_P;
+    ms.C3 = ms.OV + HEAD_OV;
+    Blk blk{reinterpret_cast<BlkScratch *>(ms.C3 + HEAD_OV), 0u, 0u};
+    // divisor prefix: limbs s_lo..k, s_lo the s of an iteration at l = HEAD_L (no head iteration reaches lower),
+    // zeros above limb k
+    const int s_lo = max(0, k - 2 * HEAD_L + 1 - 2) & ~3;
+    const int cnt = k + 1 - s_lo;
+    for (int i = lane; i < HEAD_V; i += 32) Vs[i] = (i < cnt) ? __ldg(vg + s_lo + i) : 0u;
+    __syncwarp();
+    const limb *V = Vs - s_lo;                                 // V[i] = limb i of v for i >= s_lo
+    warp_seed(V, k, Wc);
+    count(CNT_SEEDS);
+    __syncwarp();
+    int l = SEED_L, wlen = 24;
+    for (int it = SEED_ITERS; it < hp.it_end; ++it) {
+        const int m = min(H + 1 - l, l);
+        const int nlen = round_up(l + m + 2 + 2, TILE);
+        refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, true, nullptr);
+        l = l + m - 1;
+        wlen = nlen;
+        limb *t = Wc; Wc = Wn; Wn = t;
+    }
+    for (int i = lane; i < hp.wlen_end; i += 32) wrow[i] = Wc[i];
+    count_tiles(blk);
 }
 
 }  // namespace mpd

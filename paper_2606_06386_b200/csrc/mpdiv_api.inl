@@ -101,6 +101,50 @@ seed_kernel(const limb *__restrict__ v, int v_limbs, limb *__restrict__ w, int b
 }
 
 // ---------------------------------------------------------------------------------------
+// head of Refine for a whole batch: one warp (= one block) per division (mp_div.cuh "Head of Refine")
+// ---------------------------------------------------------------------------------------
+// significant limbs of a row in global memory (n a multiple of 4, row 16-byte aligned), scanned from the top
+// 512 limbs at a time with four 16-byte loads in flight per lane
+__device__ __forceinline__ int warp_prec(const limb *__restrict__ a, int n)
+{
+    const uint4 *a4 = reinterpret_cast<const uint4 *>(a);
+    const int n4 = n >> 2, lane = (int)threadIdx.x;
+    for (int hi = n4; hi > 0; hi -= 128) {
+        uint4 x[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int i = hi - 128 + 32 * j + lane;          // 16-byte word index
+            x[j] = (i >= 0) ? __ldg(a4 + i) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int j = 3; j >= 0; j--) {
+            const uint32_t nz = __ballot_sync(0xffffffffu, (x[j].x | x[j].y | x[j].z | x[j].w) != 0u);
+            if (nz) {
+                const int top_lane = 31 - __clz(nz);
+                const uint32_t xx = __shfl_sync(0xffffffffu, x[j].x, top_lane), xy = __shfl_sync(0xffffffffu, x[j].y, top_lane);
+                const uint32_t xz = __shfl_sync(0xffffffffu, x[j].z, top_lane), xw = __shfl_sync(0xffffffffu, x[j].w, top_lane);
+                const int i = hi - 128 + 32 * j + top_lane;
+                return 4 * i + (xw ? 4 : xz ? 3 : xy ? 2 : (xx ? 1 : 0));
+            }
+        }
+    }
+    return 0;
+}
+
+__global__ void __launch_bounds__(32, 16)
+shinv_head_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
+                  limb *__restrict__ wmid, int batch)
+{
+    extern __shared__ __align__(1024) uint32_t smem[];
+    const int inst = blockIdx.x;
+    if (inst >= batch) return;
+    const int h = warp_prec(u + (size_t)inst * u_limbs, u_limbs);
+    const int pv = warp_prec(v + (size_t)inst * v_limbs, v_limbs);
+    if (pv < 2 || pv > h) return;                        // zero and one-limb divisors, u < v: the division kernel's own paths
+    shinv_head_warp(v + (size_t)inst * v_limbs, pv - 1, h, smem, wmid + (size_t)inst * WMID_STRIDE);
+}
+
+// ---------------------------------------------------------------------------------------
 // shinv_batch kernel
 // ---------------------------------------------------------------------------------------
 template <int T>
@@ -158,9 +202,19 @@ constexpr int CORR_MAX = 64;
 template <int T, bool LAT>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : (T == 128 ? MPDIV_B128 : 512 / T))
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
-             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l)
+             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l,
+             const limb *__restrict__ wmid)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
+#ifdef MPDIV_STAGGER_EXPERIMENT
+    {   // tuning: delay the first-wave blocks of each SM slot by slot * stagger
+        const int stg = narrow_l >> 16;
+        if (stg && blockIdx.x < 4 * 148) {
+            const long long t0 = clock64(), wait = (long long)((blockIdx.x / 148) & 3) * stg * 1024;
+            while (clock64() - t0 < wait) { }
+        }
+    }
+#endif
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
     limb *U = smem + L.u_off;          // dividend at U + 4 (same)
     limb *WA = smem + L.wa_off;        // shinv, then the quotient
@@ -230,7 +284,8 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
         PHASE(1);
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256));
+        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256),
+                                      (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
         PHASE(2);
 
@@ -408,7 +463,43 @@ struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; 
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 // low byte: l up to which Refine runs on warp 0 alone; bit 8: MPDIV_NO_SEED (tuning: start Refine at l = 2)
-int narrow_for(int batch) { return (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0); }
+int narrow_for(int batch)
+{
+    int x = (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0);
+#ifdef MPDIV_STAGGER_EXPERIMENT
+    if (getenv("MPDIV_STAGGER")) x |= atoi(getenv("MPDIV_STAGGER")) << 16;
+#endif
+    return x;
+}
+
+// the head kernel pays off when the SMs hold several blocks each and Refine has iterations to hand over
+constexpr int HEAD_MIN_LIMBS = 512;
+static bool use_head(int u_limbs, int clip, bool lat)
+{
+    return clip && !lat && u_limbs >= HEAD_MIN_LIMBS && !getenv("MPDIV_NO_HEAD") && !getenv("MPDIV_NO_SEED");
+}
+
+// Library-owned memory pool of the current device for the head's workspace rows: freed rows stay in the pool
+// (release threshold = everything), so a call costs a pool look-up, not a driver allocation.
+static cudaMemPool_t head_pool()
+{
+    static cudaMemPool_t pools[64] = {nullptr};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    if (!pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t mp = nullptr;
+        if (cudaMemPoolCreate(&mp, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep);
+        pools[dev] = mp;
+    }
+    return pools[dev];
+}
 
 template <int T, bool LAT>
 int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
@@ -419,8 +510,22 @@ int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched));
-    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+    // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
+    // iterate over in a stream-ordered workspace (mp_div.cuh "Head of Refine")
+    limb *wmid = nullptr;
+    if (use_head(u_limbs, clip, LAT)) {
+        if (!head_pool() ||
+            cudaMallocFromPoolAsync(reinterpret_cast<void **>(&wmid), (size_t)batch * WMID_STRIDE * sizeof(limb), head_pool(), st) != cudaSuccess) {
+            cudaGetLastError();
+            wmid = nullptr;                                  // no pool on this device: Refine stays in the block
+        } else {
+            shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
+        }
+    }
+    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched), wmid);
+    const bool ok = cudaGetLastError() == cudaSuccess;
+    if (wmid) cudaFreeAsync(wmid, st);
+    return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
 // sched = the number of divisions that share the GPU with this launch (the batch itself, or the whole batch
