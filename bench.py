@@ -411,7 +411,7 @@ def run_ours(args):
                    "timing": "CUDA events per step on the launch stream, summed; max over ranks"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                 "api": "mpdiv_batch_host (pinned host buffers)", "matches_device_run": same},
-        "gpu_launches": args.steps,
+        "gpu_launches": args.steps * binding.batch_launches(m, b),
         "clocks": clocks,
         "roofline": roofline,
         "step_ms_min_median_max": [float(np.min(ms)), float(np.median(ms)), float(np.max(ms))],

@@ -189,6 +189,14 @@ int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t s
  */
 int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpdiv_stream_t stream);
 
+/*
+ * Kernels one mpdiv_batch_ex call of this shape launches: 1, or 2 when the head of Refine runs in its own
+ * kernel (clipped variant, u_limbs >= 512, more divisions than the latency-oriented kernel takes: the seed
+ * and the Refine iterations up to l = 129 then run one warp per division ahead of the division kernel and
+ * hand their iterate over in a stream-ordered workspace from a library-owned memory pool).  0 on bad arguments.
+ */
+int mpdiv_batch_launches(int u_limbs, int batch, int variant);
+
 /* "mpdiv <version> sm_100a ..." */
 const char *mpdiv_version(void);
 const char *mpdiv_strerror(int code);

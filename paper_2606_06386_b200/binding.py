@@ -55,6 +55,7 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
         L.mpdiv_debug_counters.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), i, _VOIDP]
         L.mpdiv_seed_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP]
+        L.mpdiv_batch_launches.argtypes = [i, i, i]
         L.mpdiv_version.restype = ctypes.c_char_p
         L.mpdiv_strerror.argtypes = [i]
         L.mpdiv_strerror.restype = ctypes.c_char_p
@@ -67,7 +68,7 @@ def lib() -> ctypes.CDLL:
 
 EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
-           "mpdiv_debug_counters", "mpdiv_seed_batch", "mpdiv_version", "mpdiv_strerror")
+           "mpdiv_debug_counters", "mpdiv_seed_batch", "mpdiv_batch_launches", "mpdiv_version", "mpdiv_strerror")
 
 
 def version() -> str:
@@ -171,6 +172,11 @@ def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = 
         _raise(lib().shinv_batch_ex(v.data_ptr(), v.shape[1], int(h), w.data_ptr(), w_limbs, batch, int(variant),
                                     _stream_ptr(stream)), "shinv_batch_ex")
     return w
+
+
+def batch_launches(u_limbs: int, batch: int, variant: int = VARIANT_DEFAULT) -> int:
+    """Kernels one mpdiv_batch call of this shape launches (2 when the head of Refine runs in its own kernel)."""
+    return int(lib().mpdiv_batch_launches(int(u_limbs), int(batch), int(variant)))
 
 
 SEED_LIMBS = 24     # limbs per row of mpdiv_seed_batch (20 significant)

@@ -742,6 +742,14 @@ int mpdiv_debug_phases(unsigned long long out[64], int reset)
 }
 #endif
 
+int mpdiv_batch_launches(int u_limbs, int batch, int variant)
+{
+    if (u_limbs <= 0 || batch <= 0 || !device_props()) return 0;
+    const int T = threads_for(u_limbs);
+    const bool lat = T <= 256 && batch <= (T <= 128 ? 2 : 1) * g_sm_count;
+    return use_head(u_limbs, variant == MPDIV_VARIANT_CLIPPED, lat) ? 2 : 1;
+}
+
 int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpdiv_stream_t stream)
 {
     if (!v || !w || v_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;

@@ -119,3 +119,71 @@ def test_division_same_with_and_without_seed(cfg, monkeypatch):
     torch.cuda.synchronize()
     assert binding.debug_counters()["seeds"] == 0
     assert torch.equal(q0, q1) and torch.equal(r0, r1)
+
+
+# ---- the head of Refine in its own kernel (csrc/mp_div.cuh "Head of Refine") ------------------------------
+
+def _div(u, v):
+    import torch
+
+    from paper_2606_06386_b200 import binding
+
+    du = torch.from_numpy(u.view(np.int32)).cuda()
+    dv = torch.from_numpy(v.view(np.int32)).cuda()
+    q, r = binding.mpdiv_batch(du, dv)
+    torch.cuda.synchronize()
+    return q.cpu().numpy().view(np.uint32), r.cpu().numpy().view(np.uint32)
+
+
+def test_batch_launches_reports_the_head_kernel():
+    from paper_2606_06386_b200 import binding
+
+    assert binding.batch_launches(2048, 1184) == 2            # config 2: head + division
+    assert binding.batch_launches(8192, 592) == 2
+    assert binding.batch_launches(2048, 32) == 1              # latency-oriented kernel keeps Refine in the block
+    assert binding.batch_launches(256, 100000) == 1           # below 512 limbs
+    assert binding.batch_launches(2048, 1184, binding.VARIANT_PRINTED) == 1
+    assert binding.batch_launches(0, 5) == 0
+
+
+@pytest.mark.parametrize("M,count", [(512, 1500), (1024, 900), (2048, 700), (4096, 400)])
+def test_head_kernel_random_precisions(M, count, monkeypatch):
+    """Batches large enough for the head kernel, random effective precisions of u and v: every H = h - k from
+    below the seed's threshold (17) through every split point of head_plan occurs.  q and r against the oracle,
+    and identical with the head switched off."""
+    from oracle import oracle
+    from paper_2606_06386_b200 import binding
+
+    assert binding.batch_launches(M, count) == 2
+    rng = inputs.rng_for(410, M % 65536)
+    us, vs = [], []
+    for i in range(count):
+        lv = int(rng.integers(1, M + 1))
+        if i % 4 == 0:
+            lu = min(M, lv + int(rng.integers(0, 300)))       # H around the thresholds 17, 33, 65, 129, 257
+        else:
+            lu = int(rng.integers(0, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, lv))
+    u, v = inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M)
+    binding.debug_counters(reset=True)
+    q1, r1 = _div(u, v)
+    cnt = binding.debug_counters(reset=True)
+    assert cnt["seeds"] > 0 and cnt["delta_out_of_range"] == 0
+    qo, ro = oracle.divmod_batch(u, v)
+    assert (q1 == qo).all() and (r1 == ro).all()
+    monkeypatch.setenv("MPDIV_NO_HEAD", "1")
+    q0, r0 = _div(u, v)
+    assert (q0 == q1).all() and (r0 == r1).all()
+
+
+@pytest.mark.parametrize("M,n", [(1024, 512), (2048, 1024), (2048, 2048)])
+def test_head_kernel_directed(M, n):
+    """The directed corner-case set at head-kernel batch sizes (powers of B, v = B^k + c, sparse divisors,
+    delta = -1 dividends, h - k in {0, 1, 2, 3, 2^j + 1})."""
+    from oracle import oracle
+
+    u, v = inputs.directed(M, n, count=1024, seed=inputs.SEED + 3)
+    q, r = _div(u, v)
+    qo, ro = oracle.divmod_batch(u, v)
+    assert (q == qo).all() and (r == ro).all()
