@@ -39,7 +39,9 @@ IMAD_PER_CLK_PER_SM = 64
 FLUSH_BYTES = 256 << 20   # > 126 MB of L2
 
 # DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_final.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 15372288 + 1470464, 3: 38213888 + 26464512, 4: 38073088 + 25319168}
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 16292352 + 1147904, 3: 39562752 + 24485632, 4: 38811904 + 23737856}
+# share of the division kernel in a device-resident step (the rest is the head kernel), same captures
+NCU_DIV_KERNEL_SHARE = {2: 400.2 / (400.2 + 43.6), 3: 798.4 / (798.4 + 43.6), 4: 1228.7 / (1228.7 + 40.3)}
 
 
 def parse_args():
@@ -182,11 +184,14 @@ def cpu_baseline(cfg: int, target_core_seconds: float = 16.0):
     per = (time.perf_counter() - t0) / probe            # wall seconds per division with all cores busy
     wall = target_core_seconds / cores
     count = int(max(cores, min(b, wall / max(per, 1e-9))))
-    passes = int(max(1, min(50, round(wall / max(per * count, 1e-9)))))
+    passes = 0
     t0 = time.perf_counter()
-    for _ in range(passes):
+    while True:                                         # whole passes until the core-second budget is spent
         oracle.divmod_batch(u[:count], v[:count], threads=cores)
-    dt = time.perf_counter() - t0
+        passes += 1
+        dt = time.perf_counter() - t0
+        if dt >= wall or passes >= 200:
+            break
     return {"value": passes * count / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "%d passes over the first %d of %d instances of config %d, Knuth Algorithm D (oracle/knuth_d.c), "
                       "%d host threads, %.2f s wall (%.1f core-seconds)" % (passes, count, b, cfg, cores, dt, dt * cores)}
@@ -366,7 +371,7 @@ def run_ours(args):
     if rank != 0:
         return
 
-    # ---- roofline of the dominant (only) kernel ------------------------------------------------------
+    # ---- roofline of the dominant kernel (a step = the head kernel + the division kernel, timed together) ---
     peaks = measure_imad_peak(binding)
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     nominal_peak = sm_count * IMAD_PER_CLK_PER_SM * 1965e6          # 32-bit IMAD/s at the max SM clock
@@ -390,6 +395,10 @@ def run_ours(args):
             "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
                                 "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
             "bound": "alu", "kernel": "mpdiv_kernel",
+            "kernels_per_step": binding.batch_launches(m, b),
+            "kernel_share_of_step": NCU_DIV_KERNEL_SHARE.get(cfg) if binding.batch_launches(m, b) == 2 else 1.0,
+            "timed_region": "CUDA events around the whole step (shinv_head_kernel + mpdiv_kernel on the launch stream): "
+                            "achieved and frac are per step, i.e. they charge the head kernel's time to the division",
             "achieved": achieved / 1e9, "peak": peak_products / 1e9, "unit": "G limb-products/s",
             "frac": achieved / peak_products, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg),
             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture per launch "

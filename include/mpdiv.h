@@ -54,6 +54,11 @@ enum {
  * limbs, and up to M when the divisor is short; both outputs are zero padded.
  * v_i = 0 (undefined in the paper) does not trap: q_i is set to all ones, r_i to the
  * low v_limbs limbs of u_i, and the instance is counted in mpdiv_debug_counters.
+ * Launches: one kernel, one division per thread block; a throughput batch of the clipped variant
+ * (mpdiv_batch_launches() == 2) runs the short-operand head of Refine in a kernel of its own first, one
+ * warp per division, and passes its iterate (batch x 272 limbs) through a stream-ordered allocation from a
+ * library-owned memory pool of the current device (created on first use, never destroyed; freed rows stay
+ * in the pool).  Everything is enqueued on `stream`; nothing synchronises.
  */
 int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                 uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
