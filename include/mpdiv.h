@@ -33,6 +33,15 @@
 extern "C" {
 #endif
 
+/*
+ * Tuning switches (environment, read at every launch; for A/B measurements and the tests, not for production):
+ *   MPDIV_NO_SEED=1   Refine starts at l = 2 as printed instead of the 17-digit seed (clipped variant)
+ *   MPDIV_NO_HEAD=1   the head of Refine stays inside the division kernel (see mpdiv_batch_launches)
+ *   MPDIV_NO_MMA=1    every product of the division runs on the IMAD engine (no tcgen05 range products)
+ *   MPDIV_THREADS=n   block size override (64, 128, 256, 512)
+ * None of them changes a result: q and r are exact either way.
+ */
+
 /* binary-compatible with cudaStream_t (0 / NULL = the legacy default stream) */
 typedef struct CUstream_st *mpdiv_stream_t;
 

@@ -196,25 +196,13 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // bound only has to keep |delta| * v below B^(k+2), the range of the remainder arithmetic.
 constexpr int CORR_MAX = 64;
 
-#ifndef MPDIV_B128
-#define MPDIV_B128 4      // resident 128-thread blocks per SM the register budget is set for
-#endif
 template <int T, bool LAT>
-__global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : (T == 128 ? MPDIV_B128 : 512 / T))
+__global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l,
              const limb *__restrict__ wmid)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
-#ifdef MPDIV_STAGGER_EXPERIMENT
-    {   // tuning: delay the first-wave blocks of each SM slot by slot * stagger
-        const int stg = narrow_l >> 16;
-        if (stg && blockIdx.x < 4 * 148) {
-            const long long t0 = clock64(), wait = (long long)((blockIdx.x / 148) & 3) * stg * 1024;
-            while (clock64() - t0 < wait) { }
-        }
-    }
-#endif
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
     limb *U = smem + L.u_off;          // dividend at U + 4 (same)
     limb *WA = smem + L.wa_off;        // shinv, then the quotient
@@ -463,14 +451,7 @@ struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; 
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 // low byte: l up to which Refine runs on warp 0 alone; bit 8: MPDIV_NO_SEED (tuning: start Refine at l = 2)
-int narrow_for(int batch)
-{
-    int x = (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0);
-#ifdef MPDIV_STAGGER_EXPERIMENT
-    if (getenv("MPDIV_STAGGER")) x |= atoi(getenv("MPDIV_STAGGER")) << 16;
-#endif
-    return x;
-}
+int narrow_for(int batch) { return (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0); }
 
 // the head kernel pays off when the SMs hold several blocks each and Refine has iterations to hand over
 constexpr int HEAD_MIN_LIMBS = 512;
