@@ -248,7 +248,7 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
         s.clear();
         int I = Ilo + c;
         if (I <= Ihi) {
-            tiles += (uint32_t)(Ihi - I) / (uint32_t)C + 1u;
+            tiles += ((uint32_t)(Ihi - I) >> sh) + 1u;
             uint32_t a0[8], b0[8], a1[8], b1[8];
             const int step = 4 * TILE * C;                  // bytes between a lane's consecutive tiles
             uint32_t pa = (uint32_t)__cvta_generic_to_shared(A) + 4 * TILE * I;
