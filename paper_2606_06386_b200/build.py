@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmpdiv.so")
 SOURCES = ["mpdiv.cu"]
-DEPS = ["mpdiv.cu", "mp_block.cuh", "mp_mul.cuh", "mp_div.cuh", "mpdiv_api.inl",
+DEPS = ["mpdiv.cu", "mp_block.cuh", "mp_mul.cuh", "mp_mma.cuh", "mp_div.cuh", "mpdiv_api.inl",
         os.path.join("..", "..", "include", "mpdiv.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -32,6 +32,7 @@
 // for full 1024 / 2048 / 4096-limb squares against 9.15e12 for the IMAD.WIDE roofline probe.  One
 // `tcgen05.mma` (M = 128, K = 32, u8) takes about 132 cycles whatever N <= 256 is.
 #pragma once
+#include <type_traits>
 #include "mp_block.cuh"
 
 namespace mpd {
@@ -62,6 +63,15 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity)
         if (ok) return true;
     }
     return false;
+}
+// one lane of a converged warp (elect.sync): the branch it guards is uniform for ptxas, so the tcgen05
+// instructions inside are issued straight from uniform registers -- under `if (tid == X)` every
+// tcgen05.mma / tcgen05.commit is wrapped in an ELECT / BRA.U.ANY loop over the "possibly several" active lanes
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -307,24 +317,38 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     using Roles = MmaRoles<T>;
     constexpr int G = Roles::GROUPS;
     const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
-    // the MMAs of one step: D[:, 0..Nn) += A_p x B_p (K = 128 as four instructions of K = 32)
-    auto issue_step = [&](int step) -> bool {
+    // the MMAs of one step: D[:, 0..Nn) += A_p x B_p (K = 128 as four instructions of K = 32), then the commit that
+    // frees the step's Toeplitz stage s.  WARP = true: called by a whole converged warp, one elected lane issues
+    // (the election sits directly around the straight-line tcgen05 code: with a loop inside the elected region
+    // ptxas falls back to its ELECT / BRA.U.ANY loop around every instruction); false: called by one thread.
+    auto issue_mmas = [&](int step, int s, auto warp_form) {
+        constexpr bool WARP = decltype(warp_form)::value;
         const int p = pmin + step;
-        const uint32_t t = cx.it + (uint32_t)step;
-        const int s = Roles::stage(t);
-        if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) return false;
-        tc_fence_after();
         const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
         for (int nc = 0; nc < Nn; nc += 256) {
             const int ncols = min(256, Nn - nc);
             const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
             const uint32_t idesc = mma_idesc(ncols);
+            bool lead = true;
+            if constexpr (WARP) lead = elect_one();
+            if (lead) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
-                             (step > 0 || k > 0) ? 1u : 0u);
+                for (int k = 0; k < 4; ++k)
+                    tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
+                                 (step > 0 || k > 0) ? 1u : 0u);
+            }
         }
-        tc_commit(cx.bar + 64 + 8 * s);
+        bool lead = true;
+        if constexpr (WARP) lead = elect_one();
+        if (lead) tc_commit(cx.bar + 64 + 8 * s);
+    };
+    // a step issued by a single thread of a diverged warp (COMBINED blocks)
+    auto issue_step = [&](int step) -> bool {
+        const uint32_t t = cx.it + (uint32_t)step;
+        const int s = Roles::stage(t);
+        if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) return false;
+        tc_fence_after();
+        issue_mmas(step, s, std::false_type{});
         return true;
     };
     if (warp < 4 * G) {
@@ -348,11 +372,18 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
             if (Roles::COMBINED && tid == Roles::ISSUER && !issue_step(step)) { cx.fail = 2; break; }
         }
         if (Roles::COMBINED && tid == Roles::ISSUER) tc_commit(cx.bar + 128);
-    } else if (!Roles::COMBINED && tid == Roles::ISSUER) {
-        // ---- the MMA issuer ----
-        for (int step = 0; step < nsteps; ++step)
-            if (!issue_step(step)) { cx.fail = 2; break; }
-        tc_commit(cx.bar + 128);
+    } else if (!Roles::COMBINED && warp == Roles::ISSUER / 32) {
+        // ---- the MMA issuer: the whole warp walks the steps (uniform control flow), one elected lane issues ----
+        for (int step = 0; step < nsteps; ++step) {
+            const uint32_t t = cx.it + (uint32_t)step;
+            const int s = Roles::stage(t);
+            if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) { cx.fail = 2; break; }
+            tc_fence_after();
+            issue_mmas(step, s, std::true_type{});
+            __syncwarp();
+        }
+        if (elect_one()) tc_commit(cx.bar + 128);
+        __syncwarp();
     }
     cx.it += (uint32_t)nsteps;
     __syncwarp();

@@ -714,6 +714,14 @@ int mpdiv_debug_phases(unsigned long long out[64], int reset)
     if (cudaMemcpyFromSymbol(op, g_op, sizeof(op)) != cudaSuccess) return MPDIV_ERR_CUDA;
     for (int i = 0; i < 8; i++) out[8 + i] = op[i];      // slots 8..15: op-level split of Refine iterations 0..5
     if (reset) { unsigned long long zz[16] = {0}; cudaMemcpyToSymbol(g_op, zz, sizeof(zz)); }
+#ifdef MMA_TIMING
+    {   // slots 56..63: tensor-core multiplier sub-phases (row operand, MMA loop, wait, epilogue, final add)
+        unsigned long long mt[8];
+        if (cudaMemcpyFromSymbol(mt, g_mma_t, sizeof(mt)) != cudaSuccess) return MPDIV_ERR_CUDA;
+        for (int i = 0; i < 8; i++) out[56 + i] = mt[i];
+        if (reset) { unsigned long long zz[8] = {0}; cudaMemcpyToSymbol(g_mma_t, zz, sizeof(zz)); }
+    }
+#endif
     if (reset) {
         unsigned long long z[64] = {0};
         if (cudaMemcpyToSymbol(g_phase, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
