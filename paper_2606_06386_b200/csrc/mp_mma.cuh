@@ -98,6 +98,21 @@ __device__ __forceinline__ void tc_mma_i8_ts(uint32_t tmem_d, uint32_t tmem_a, u
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}"
                  ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
 }
+// same with the shared-memory descriptor given by its low word (mma_desc_lo); the high word is the constant
+// part of mma_smem_desc.  The issuer prepares the words in ordinary registers BEFORE it elects its lane, so
+// that the elected path is R2UR + tcgen05.mma only (arithmetic on the uniform datapath sits on the issue path:
+// a chain R2UR - UIADD3 - USHF - ULOP3 - ULOP3 in front of every instruction cost ~120 cycles per MMA against
+// a tensor-core time of N / 2 cycles)
+constexpr uint32_t MMA_DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+__device__ __forceinline__ uint32_t mma_desc_lo(uint32_t saddr) { return ((saddr >> 4) & 0x3FFFu) | (1u << 16); }
+__device__ __forceinline__ void tc_mma_i8_ts_lo(uint32_t tmem_d, uint32_t tmem_a, uint32_t bdesc_lo, uint32_t idesc,
+                                                uint32_t accumulate)
+{
+    const uint32_t z = 0;
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 bd;\n\tsetp.ne.b32 p, %4, 0;\n\tmov.b64 bd, {%2, %6};\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], bd, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "r"(tmem_a), "r"(bdesc_lo), "r"(idesc), "r"(accumulate), "r"(z), "r"(MMA_DESC_HI) : "memory");
+}
 // 32 lanes x 32 columns: each thread of the warp stores its 32 registers into its own lane
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
 {
@@ -317,29 +332,40 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     using Roles = MmaRoles<T>;
     constexpr int G = Roles::GROUPS;
     const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
-    // the MMAs of one step: D[:, 0..Nn) += A_p x B_p (K = 128 as four instructions of K = 32), then the commit that
-    // frees the step's Toeplitz stage s.  WARP = true: called by a whole converged warp, one elected lane issues
-    // (the election sits directly around the straight-line tcgen05 code: with a loop inside the elected region
-    // ptxas falls back to its ELECT / BRA.U.ANY loop around every instruction); false: called by one thread.
-    auto issue_mmas = [&](int step, int s, auto warp_form) {
+    // MMAs k0 <= k < k1 of one step for the accumulator columns nc .. nc+255: D[:, nc..] += A_p x B_p, K = 128 as
+    // four instructions of K = 32.  WARP = true: called by a whole converged warp, one elected lane issues (the
+    // election sits directly around the straight-line tcgen05 code: with a loop inside the elected region ptxas
+    // falls back to its ELECT / BRA.U.ANY loop around every instruction); false: called by one thread.
+    auto issue_mmas = [&](int step, int s, int nc, int k0, int k1, auto warp_form) {
         constexpr bool WARP = decltype(warp_form)::value;
         const int p = pmin + step;
-        const uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
-        for (int nc = 0; nc < Nn; nc += 256) {
-            const int ncols = min(256, Nn - nc);
-            const uint32_t b_addr = smem_u32(cx.brows + (dlo + nc - p - e0) * 128);
-            const uint32_t idesc = mma_idesc(ncols);
-            bool lead = true;
-            if constexpr (WARP) lead = elect_one();
-            if (lead) {
+        uint32_t d_tmem = cx.tmem_base + (uint32_t)nc;
+        uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
+        uint32_t b_lo = mma_desc_lo(smem_u32(cx.brows + (dlo + nc - p - e0) * 128));   // + 2 per K slice of 32 bytes
+        uint32_t idesc = mma_idesc(min(256, Nn - nc));
+        uint32_t acc0 = (step > 0 || k0 > 0) ? 1u : 0u;
+        uint32_t ak[4], bk[4];
 #pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    tc_mma_i8_ts(cx.tmem_base + nc, a_tmem + 8 * k, mma_smem_desc(b_addr + 32 * k), idesc,
-                                 (step > 0 || k > 0) ? 1u : 0u);
-            }
+        for (int k = 0; k < 4; ++k) { ak[k] = a_tmem + 8 * k; bk[k] = b_lo + 2 * k; }
+        if constexpr (WARP) {
+            // every lane computes the operand words; the empty asm keeps the arithmetic out of the elected branch
+            asm volatile("" : "+r"(d_tmem), "+r"(idesc), "+r"(acc0));
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (k >= k0 && k < k1) asm volatile("" : "+r"(ak[k]), "+r"(bk[k]));
         }
         bool lead = true;
         if constexpr (WARP) lead = elect_one();
+        if (lead) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (k >= k0 && k < k1) tc_mma_i8_ts_lo(d_tmem, ak[k], bk[k], idesc, k == k0 ? acc0 : 1u);
+        }
+    };
+    // the commit that frees the step's Toeplitz stage s
+    auto commit_stage = [&](int s, auto warp_form) {
+        bool lead = true;
+        if constexpr (decltype(warp_form)::value) lead = elect_one();
         if (lead) tc_commit(cx.bar + 64 + 8 * s);
     };
     // a step issued by a single thread of a diverged warp (COMBINED blocks)
@@ -348,7 +374,8 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         const int s = Roles::stage(t);
         if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) return false;
         tc_fence_after();
-        issue_mmas(step, s, std::false_type{});
+        for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::false_type{});
+        commit_stage(s, std::false_type{});
         return true;
     };
     if (warp < 4 * G) {
@@ -373,14 +400,23 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         }
         if (Roles::COMBINED && tid == Roles::ISSUER) tc_commit(cx.bar + 128);
     } else if (!Roles::COMBINED && warp == Roles::ISSUER / 32) {
-        // ---- the MMA issuer: the whole warp walks the steps (uniform control flow), one elected lane issues ----
+        // ---- the MMA issuer: the whole warp walks the steps (uniform control flow), one elected lane issues.
+        // The wait for the NEXT step's tile sits between the second and third MMA of a step: the issue of an MMA
+        // blocks while the tensor core's queue is full, so everything between two steps (commit, barrier poll,
+        // fence, descriptors) would otherwise run with a single MMA left in flight.
+        bool ok = mbar_wait(cx.bar + 8 * Roles::stage(cx.it), Roles::use(cx.it) & 1);
         for (int step = 0; step < nsteps; ++step) {
-            const uint32_t t = cx.it + (uint32_t)step;
-            const int s = Roles::stage(t);
-            if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) { cx.fail = 2; break; }
+            if (!ok) { cx.fail = 2; break; }
+            const int s = Roles::stage(cx.it + (uint32_t)step);
             tc_fence_after();
-            issue_mmas(step, s, std::true_type{});
-            __syncwarp();
+            issue_mmas(step, s, 0, 0, 2, std::true_type{});
+            if (step + 1 < nsteps) {
+                const uint32_t tn = cx.it + (uint32_t)step + 1u;
+                ok = mbar_wait(cx.bar + 8 * Roles::stage(tn), Roles::use(tn) & 1);
+            }
+            issue_mmas(step, s, 0, 2, 4, std::true_type{});
+            for (int nc = 256; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
+            commit_stage(s, std::true_type{});
         }
         if (elect_one()) tc_commit(cx.bar + 128);
         __syncwarp();
