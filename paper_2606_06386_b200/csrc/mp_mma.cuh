@@ -401,22 +401,34 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         if (Roles::COMBINED && tid == Roles::ISSUER) tc_commit(cx.bar + 128);
     } else if (!Roles::COMBINED && warp == Roles::ISSUER / 32) {
         // ---- the MMA issuer: the whole warp walks the steps (uniform control flow), one elected lane issues.
-        // The wait for the NEXT step's tile sits between the second and third MMA of a step: the issue of an MMA
-        // blocks while the tensor core's queue is full, so everything between two steps (commit, barrier poll,
-        // fence, descriptors) would otherwise run with a single MMA left in flight.
-        bool ok = mbar_wait(cx.bar + 8 * Roles::stage(cx.it), Roles::use(cx.it) & 1);
+        // The warp's own instructions are the critical path (a tensor-core step takes 2 N cycles, 256 for N = 128),
+        // so the loop carries the stage index, the barrier parity and the operand words incrementally (no
+        // division by GROUPS per step) and the elected region of a step holds its MMAs and its commit.
+        uint32_t tg = cx.it % (uint32_t)G, tq = cx.it / (uint32_t)G;              // tile t = tq * G + tg
+        uint32_t b_lo0 = mma_desc_lo(smem_u32(cx.brows + (dlo - pmin - e0) * 128));   // row of column 0 at step 0
+        const uint32_t idesc0 = mma_idesc(min(256, Nn));
         for (int step = 0; step < nsteps; ++step) {
-            if (!ok) { cx.fail = 2; break; }
-            const int s = Roles::stage(cx.it + (uint32_t)step);
+            const int s = (int)tg * Roles::PER_GROUP + (int)(tq % Roles::PER_GROUP);
+            if (!mbar_wait(cx.bar + 8 * s, (tq / Roles::PER_GROUP) & 1)) { cx.fail = 2; break; }
             tc_fence_after();
-            issue_mmas(step, s, 0, 0, 2, std::true_type{});
-            if (step + 1 < nsteps) {
-                const uint32_t tn = cx.it + (uint32_t)step + 1u;
-                ok = mbar_wait(cx.bar + 8 * Roles::stage(tn), Roles::use(tn) & 1);
+            uint32_t d_tmem = cx.tmem_base, a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s), b_lo = b_lo0;
+            uint32_t idesc = idesc0, acc0 = step > 0 ? 1u : 0u, ebar = cx.bar + 64 + 8 * s;
+            // every lane computes the operand words; the empty asm keeps the arithmetic out of the elected branch
+            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(acc0), "+r"(ebar));
+            if (Nn <= 256) {
+                if (elect_one()) {
+                    tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, acc0);
+                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
+                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
+                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
+                    tc_commit(ebar);
+                }
+            } else {
+                for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
+                commit_stage(s, std::true_type{});
             }
-            issue_mmas(step, s, 0, 2, 4, std::true_type{});
-            for (int nc = 256; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
-            commit_stage(s, std::true_type{});
+            b_lo0 -= 8u;                                         // the next step starts one 128-byte row lower
+            if (++tg == (uint32_t)G) { tg = 0; ++tq; }
         }
         if (elect_one()) tc_commit(cx.bar + 128);
         __syncwarp();
