@@ -95,7 +95,10 @@ struct ShinvBufs {
 
 // Block sizes whose kernels carry the tensor-core multiplier (mp_mma.cuh); the others never see an MmaCtx.
 template <int T>
-struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256); };   // measured: no gain at 128 threads (2^16 bits)
+struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256 || T == 128); };
+// (128-thread blocks, 2^16 bits: no gain while the MMAs were issued by a single thread of a diverged warp; +23 % at
+// config 2 with the warp-issued loop of mp_mma.cuh.  The latency kernel of small batches keeps the IMAD path:
+// launch_div_k gives it no tensor-core scratch.)
 
 // Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
 // P[i] = limb 32*dlo + i.

@@ -18,19 +18,24 @@
 //     from registers into TENSOR MEMORY (`tcgen05.st`, lane = row, 32 columns = 128 bytes of K) and the
 //     MMA takes its A operand from there (`tcgen05.mma [d], [a_tmem], b_desc`): the tile never touches
 //     shared memory, whose bandwidth was the limit of a first version that staged A tiles in a 16 KB ring
-//     (about 840 cycles per step).  With A in tensor memory a step takes 690 cycles, which is the rate of
-//     the TS-form MMA itself (172 cycles per instruction against 132 with A in shared memory, measured with
-//     the waits removed).  Stages of 32 TMEM columns are handed to the single MMA-issuing thread through
+//     (about 840 cycles per step).  Stages of 32 TMEM columns are handed to the MMA-issuing warp through
 //     mbarriers and freed by `tcgen05.commit`.
+//   * The issuing warp's own instruction stream is the critical path of the loop.  One `tcgen05.mma` (M = 128,
+//     K = 32, u8) occupies the tensor core for max(~48, N / 2) cycles (measured: two warps issuing to disjoint
+//     accumulators reach N / 2 per instruction together; one lean warp 48 cycles at N <= 64, 64 at N = 128),
+//     but a first version issued from `if (tid == ISSUER)`, where ptxas wraps every tcgen05 instruction in an
+//     ELECT / BRA.U.ANY loop and builds each descriptor on the uniform datapath after the R2UR: 170 cycles per
+//     instruction whatever N was (690 per step).  Now the whole issuer warp walks the steps, the operand words
+//     are prepared in ordinary registers and one elected lane issues the four MMAs and the commit of a step:
+//     ~330 cycles per step at N = 128 (tensor-core time 256), ~500 at N = 256 (tensor-core time 512).
 //   * Epilogue: `tcgen05.ld` (lane = i, column = d), four adjacent lanes form one limb's 64-bit column
 //     sum, low words go to P, high words to HI one limb up, and one block-wide carry-propagating add
 //     (mp_block.cuh) finishes.
 // A range of output blocks dlo <= d < dhi can be asked for (clipped products); what is omitted below
 // block dlo is less than B^(32 dlo + 1).  Only steps p whose chunk d - p can be non-zero are issued.
 //
-// Measured on B200 (standalone, one product per SM at a time): 1.07e13 / 2.3e13 / 4.3e13 limb products/s
-// for full 1024 / 2048 / 4096-limb squares against 9.15e12 for the IMAD.WIDE roofline probe.  One
-// `tcgen05.mma` (M = 128, K = 32, u8) takes about 132 cycles whatever N <= 256 is.
+// Measured on B200 (mpmul_batch_ex, whole batches): 592 full 4096 x 4096-limb products in 0.245 ms = 4.1e13
+// limb products/s against 9.15e12 for the IMAD.WIDE roofline probe; 1184 x (2048 x 2048) in 0.226 ms.
 #pragma once
 #include <type_traits>
 #include "mp_block.cuh"
@@ -265,11 +270,11 @@ __device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
     return min(Ea, dhi - 1) - max(0, dlo - Eb + 1) + 1;
 }
 
-// Should this range product run on the tensor core?  Measured on B200 (512-thread block alone on its SM):
-// a step costs about 600 cycles (four MMA instructions of ~132 cycles whatever N is, plus hand-over), a call
-// about 12 000 cycles of fixed work (row operand,
-// epilogue, final add), against about 1/26 cycle per limb product on the IMAD path.  swap = take b as the
-// Toeplitz operand (fewer steps).  Block-uniform.
+// Should this range product run on the tensor core?  Cost model in cycles of a block alone on its SM: a step
+// (four MMA instructions) is entered as 700 cycles and a call as 12 000 cycles of fixed work (row operand,
+// epilogue, final add), against about 1/26 cycle per limb product on the IMAD path; MMA_PLAN_PCT scales the
+// tensor side to what is measured (a step of the warp-issued loop takes ~330 cycles at N <= 144).  swap = take
+// b as the Toeplitz operand (fewer steps).  Block-uniform.
 template <int T>
 __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
 {
@@ -284,7 +289,8 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
     // the IMAD path of a block of T threads gets T/512 of the SM's 26 limb products per cycle
 #ifndef MMA_PLAN_PCT
-#define MMA_PLAN_PCT 35     // measured: the model below is pessimistic for the tensor path; 35 % is +1-2 % at 2^17, 2^18 bits
+#define MMA_PLAN_PCT 10     // measured (sweep 3..35 with the warp-issued MMA loop, ~330 cycles per step): 10 % is best at 2^17
+                            // bits and within 1 % of the best (6 %) at 2^18 bits; 35 % was the optimum of the thread-issued loop
 #endif
     return 100 * est >= (long long)(MMA_PLAN_PCT * 52 * T / 512) * (700ll * steps + 12000ll);
 }
@@ -336,6 +342,7 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     // four instructions of K = 32.  WARP = true: called by a whole converged warp, one elected lane issues (the
     // election sits directly around the straight-line tcgen05 code: with a loop inside the elected region ptxas
     // falls back to its ELECT / BRA.U.ANY loop around every instruction); false: called by one thread.
+    // Only products wider than 256 output blocks come here; the common case is inlined in warp_issue.
     auto issue_mmas = [&](int step, int s, int nc, int k0, int k1, auto warp_form) {
         constexpr bool WARP = decltype(warp_form)::value;
         const int p = pmin + step;
@@ -368,16 +375,32 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         if constexpr (decltype(warp_form)::value) lead = elect_one();
         if (lead) tc_commit(cx.bar + 64 + 8 * s);
     };
-    // a step issued by a single thread of a diverged warp (COMBINED blocks)
-    auto issue_step = [&](int step) -> bool {
-        const uint32_t t = cx.it + (uint32_t)step;
-        const int s = Roles::stage(t);
-        if (!mbar_wait(cx.bar + 8 * s, Roles::use(t) & 1)) return false;
+    // One step issued by a whole converged warp: poll the tile's `full` barrier (stage s, parity par), then one
+    // elected lane issues the MMAs and the commit.  b_lo = descriptor word of the row that column 0 reads at this
+    // step.  The warp's own instructions are the critical path of the MMA loop (a tensor-core step takes 2 N
+    // cycles, 256 for N = 128), so the operand words are prepared by every lane in ordinary registers (the empty
+    // asm keeps the arithmetic out of the elected branch) and the elected region is straight-line code.
+    auto warp_issue = [&](int step, int s, uint32_t par, uint32_t b_lo) -> bool {
+        if (!mbar_wait(cx.bar + 8 * s, par)) return false;
         tc_fence_after();
-        for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::false_type{});
-        commit_stage(s, std::false_type{});
+        if (Nn <= 256) {
+            uint32_t d_tmem = cx.tmem_base, a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
+            uint32_t idesc = mma_idesc(Nn), acc0 = step > 0 ? 1u : 0u, ebar = cx.bar + 64 + 8 * s;
+            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(acc0), "+r"(ebar));
+            if (elect_one()) {
+                tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, acc0);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
+                tc_commit(ebar);
+            }
+        } else {
+            for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
+            commit_stage(s, std::true_type{});
+        }
         return true;
     };
+    const uint32_t b_lo_first = mma_desc_lo(smem_u32(cx.brows + (dlo - pmin - e0) * 128));   // step 0, column 0
     if (warp < 4 * G) {
         // ---- Toeplitz producers: warp j fills lanes 32 (j % 4) .. +31 of the tiles of group j / 4 ----
         const int grp = warp >> 2, row = tid & 127;
@@ -396,38 +419,22 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
             tc_fence_before();
             __syncwarp();
             if ((tid & 31) == 0) mbar_arrive(cx.bar + 8 * s);
-            if (Roles::COMBINED && tid == Roles::ISSUER && !issue_step(step)) { cx.fail = 2; break; }
+            if (Roles::COMBINED && warp == 0 &&            // 128-thread blocks: warp 0 also issues the step
+                !warp_issue(step, s, use & 1, b_lo_first - 8u * (uint32_t)step)) { cx.fail = 2; break; }
         }
-        if (Roles::COMBINED && tid == Roles::ISSUER) tc_commit(cx.bar + 128);
+        if (Roles::COMBINED && warp == 0) {
+            if (elect_one()) tc_commit(cx.bar + 128);
+            __syncwarp();
+        }
     } else if (!Roles::COMBINED && warp == Roles::ISSUER / 32) {
-        // ---- the MMA issuer: the whole warp walks the steps (uniform control flow), one elected lane issues.
-        // The warp's own instructions are the critical path (a tensor-core step takes 2 N cycles, 256 for N = 128),
-        // so the loop carries the stage index, the barrier parity and the operand words incrementally (no
-        // division by GROUPS per step) and the elected region of a step holds its MMAs and its commit.
+        // ---- the MMA issuer: the whole warp walks the steps (uniform control flow); stage index, barrier parity
+        // and descriptor word are carried incrementally (no division by GROUPS per step)
         uint32_t tg = cx.it % (uint32_t)G, tq = cx.it / (uint32_t)G;              // tile t = tq * G + tg
-        uint32_t b_lo0 = mma_desc_lo(smem_u32(cx.brows + (dlo - pmin - e0) * 128));   // row of column 0 at step 0
-        const uint32_t idesc0 = mma_idesc(min(256, Nn));
+        uint32_t b_lo = b_lo_first;
         for (int step = 0; step < nsteps; ++step) {
             const int s = (int)tg * Roles::PER_GROUP + (int)(tq % Roles::PER_GROUP);
-            if (!mbar_wait(cx.bar + 8 * s, (tq / Roles::PER_GROUP) & 1)) { cx.fail = 2; break; }
-            tc_fence_after();
-            uint32_t d_tmem = cx.tmem_base, a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s), b_lo = b_lo0;
-            uint32_t idesc = idesc0, acc0 = step > 0 ? 1u : 0u, ebar = cx.bar + 64 + 8 * s;
-            // every lane computes the operand words; the empty asm keeps the arithmetic out of the elected branch
-            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(acc0), "+r"(ebar));
-            if (Nn <= 256) {
-                if (elect_one()) {
-                    tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, acc0);
-                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
-                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
-                    tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
-                    tc_commit(ebar);
-                }
-            } else {
-                for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
-                commit_stage(s, std::true_type{});
-            }
-            b_lo0 -= 8u;                                         // the next step starts one 128-byte row lower
+            if (!warp_issue(step, s, (tq / Roles::PER_GROUP) & 1, b_lo)) { cx.fail = 2; break; }
+            b_lo -= 8u;                                          // the next step starts one 128-byte row lower
             if (++tg == (uint32_t)G) { tg = 0; ++tq; }
         }
         if (elect_one()) tc_commit(cx.bar + 128);

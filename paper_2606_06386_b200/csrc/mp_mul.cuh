@@ -255,25 +255,18 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
             uint32_t pb = (uint32_t)__cvta_generic_to_shared(Bp) + 4 * TILE * (K - I);
             load_tile(a0, pa);
             load_tile(b0, pb);
-            // two tiles per trip with ping-pong operand registers (no register copies); the loads of the
-            // loop are unconditional and the last pair is peeled
-            for (; I + 2 * C <= Ihi; I += 2 * C) {
+            // two tiles per trip with ping-pong operand registers (no register copies)
+            for (; I + C <= Ihi; I += 2 * C) {
                 pa += step; pb -= step;
                 load_tile(a1, pa);
                 load_tile(b1, pb);
                 tile_mac(s, a0, b0);
-                pa += step; pb -= step;
-                load_tile(a0, pa);
-                load_tile(b0, pb);
+                if (I + 2 * C <= Ihi) {
+                    pa += step; pb -= step;
+                    load_tile(a0, pa);
+                    load_tile(b0, pb);
+                }
                 tile_mac(s, a1, b1);
-            }
-            if (I + C <= Ihi) {
-                pa += step; pb -= step;
-                load_tile(a1, pa);
-                load_tile(b1, pb);
-                tile_mac(s, a0, b0);
-                tile_mac(s, a1, b1);
-                I += 2 * C;
             }
             if (I <= Ihi) tile_mac(s, a0, b0);
         }
