@@ -386,12 +386,13 @@ def run_ours(args):
         roofline = {
             "note": "achieved = W(M) x batch / t with W(M) the limb products of the method AS PRINTED (SURVEY 8(d)); the "
                     "default (clipped) variant skips the low part of w*x and u*shinv, the low and high parts of v'w and the "
-                    "high part of v*q (PAPER.md:507, :542), so frac may exceed 1; pipe_frac counts what really ran",
+                    "high part of v*q (PAPER.md:507, :542), so frac may exceed 1; pipe_frac counts the limb products that "
+                    "really ran on the IMAD pipe (the products that ran on the tensor cores are not in it)",
             "executed_limb_products_per_launch": executed,
             "pipe_frac": executed / (kernel_ms * 1e-3) / peak_products,
-            "tensor_engine": "range products with enough work (u*shinv, v*q and the last doubling Refine step at "
-                             "2^18 bits) run as int8 tcgen05 GEMMs (csrc/mp_mma.cuh); per_config times both engines "
-                             "on the same products",
+            "tensor_engine": "range products with enough work (u*shinv, v*q and the last Refine steps) run as int8 "
+                             "tcgen05 GEMMs (csrc/mp_mma.cuh) in throughput batches from 2^16 bits up; per_config times "
+                             "both engines on the same products",
             "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
                                 "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
             "bound": "alu", "kernel": "mpdiv_kernel",

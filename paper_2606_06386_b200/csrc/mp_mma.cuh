@@ -292,7 +292,10 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
 #define MMA_PLAN_PCT 10     // measured (sweep 3..35 with the warp-issued MMA loop, ~330 cycles per step): 10 % is best at 2^17
                             // bits and within 1 % of the best (6 %) at 2^18 bits; 35 % was the optimum of the thread-issued loop
 #endif
-    return 100 * est >= (long long)(MMA_PLAN_PCT * 52 * T / 512) * (700ll * steps + 12000ll);
+    // 128-thread blocks share their SM with three others and their warp 0 both produces and issues: the sweep
+    // there gives 20-30 % (config 2: 3.57 M div/s against 3.28 M at 10 % and 3.50 M at 45-70 %)
+    constexpr int pct = (T <= 128) ? 25 : MMA_PLAN_PCT;
+    return 100 * est >= (long long)(pct * 52 * T / 512) * (700ll * steps + 12000ll);
 }
 
 // P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).

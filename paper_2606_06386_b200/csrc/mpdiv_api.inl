@@ -487,8 +487,9 @@ int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
                  cudaStream_t st, int clip, int sched)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    // (a latency-bound batch of 128-thread blocks is faster on the IMAD path alone: config 1 72 us against 100 us)
-    if (MmaEnabled<T>::value && clip && !(LAT && T <= 128) && !getenv("MPDIV_NO_MMA"))
+    // (128-thread blocks: a latency-bound batch is faster on the IMAD path alone -- config 1 72 us against 100 us --
+    // and so are throughput batches of 2^15 bits, 7.07 M against 6.64 M div/s)
+    if (MmaEnabled<T>::value && clip && !(T <= 128 && (LAT || u_limbs < 1536)) && !getenv("MPDIV_NO_MMA"))
         div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
