@@ -98,15 +98,15 @@ template <int T>
 struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256 || T == 128); };
 // (128-thread blocks, 2^16 bits: no gain while the MMAs were issued by a single thread of a diverged warp; +23 % at
 // config 2 with the warp-issued loop of mp_mma.cuh.  The latency kernel of small batches keeps the IMAD path:
-// launch_div_k gives it no tensor-core scratch.)
+// its instantiation carries no tensor-core code: MMA template flag of shinv_block / refine_step / try_mma_range.)
 
 // Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
 // P[i] = limb 32*dlo + i.
-template <int T>
+template <int T, bool MMA = MmaEnabled<T>::value>
 __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na, const limb *Bp, int nb, int dlo, int dhi,
                                              limb *P, limb *HI, Blk &blk)
 {
-    if constexpr (MmaEnabled<T>::value) {
+    if constexpr (MMA) {
         bool swap;
         if (mma_plan<T>(mma, na, nb, dlo, dhi, swap))
             return swap ? mma_mul_range<T>(*mma, Bp, nb, A, na, dlo, dhi, P, HI, blk)
@@ -119,7 +119,7 @@ __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na,
 // the whole block (TT = T) or, for the early iterations whose operands are a few tiles long, warp 0 alone
 // (TT = 32: warp-level barriers only; the other warps wait at the block barrier that ends the narrow phase
 // and leave their issue slots to the other blocks of the SM).
-template <int TT>
+template <int TT, bool MMA = false>
 __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it, int l, int wlen, limb *Wc, limb *Wn,
                                             limb *X, limb *P, const MulScratch &ms, Blk &blk, bool clip, MmaCtx *mma)
 {
@@ -173,7 +173,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
             // clipped close product: limbs [c, L) of v'w only; X holds x / B^c (low limbs taken as 0)
             count(CNT_CLIPPED_STEPS);
             const int dlo = (cx - 1) / 32;               // tensor-core form: blocks of 32 limbs, E < B^(32 dlo + 1)
-            if (try_mma_range<TT>(mma, Vp, pv, Wc, pw, dlo, (L + 31) / 32, P, ms.HI, blk) >= 0) {
+            if (try_mma_range<TT, MMA>(mma, Vp, pv, Wc, pw, dlo, (L + 31) / 32, P, ms.HI, blk) >= 0) {
                 c = 32 * dlo;
                 count(CNT_MMA_PRODUCTS);
             } else {
@@ -206,7 +206,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         bool exact = (Klo1 == 0 && c == 0);
         if (clip && dd >= 33) {
             const int dlo = (dd - 1) / 32;
-            tl = try_mma_range<TT>(mma, Wc, pw, X, xl, dlo, 1 << 20, P, ms.HI, blk);
+            tl = try_mma_range<TT, MMA>(mma, Wc, pw, X, xl, dlo, 1 << 20, P, ms.HI, blk);
             if (tl >= 0) { off = dd - 32 * dlo; exact = false; count(CNT_MMA_PRODUCTS); }
         }
         if (tl >= 0) {
@@ -377,7 +377,7 @@ __device__ __forceinline__ HeadPlan head_plan(int H, int iters)
 
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
-template <int T>
+template <int T, bool MMA = false>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
                                            bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true,
                                            const limb *wmid = nullptr)
@@ -463,7 +463,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                 __syncthreads();
                 blk.parity = 0;
             }
-            refine_step<T>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, mma);
+            refine_step<T, MMA>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, mma);
         }
         l = l + m - 1;
         wlen = nlen;

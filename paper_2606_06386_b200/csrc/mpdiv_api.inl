@@ -196,6 +196,11 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
 // bound only has to keep |delta| * v below B^(k+2), the range of the remainder arithmetic.
 constexpr int CORR_MAX = 64;
 
+// Which division kernels carry the tensor-core engine: a latency-bound batch of 128-thread blocks is faster on the
+// IMAD path alone (config 1: 68 us against 100 us per division), and without the engine's code in the kernel.
+template <int T, bool LAT>
+struct DivMma { static constexpr bool value = MmaEnabled<T>::value && !(LAT && T <= 128); };
+
 template <int T, bool LAT>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
@@ -215,9 +220,11 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     mq.OV = mq.HI + L.p_words_q;
     mq.C3 = mq.OV + round_up(L.p_words_q / TILE, 4);
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
+    // the latency kernel of 128-thread blocks is compiled without the tensor-core engine (DivMma)
+    constexpr bool MMA = DivMma<T, LAT>::value;
     MmaCtx mcx;
     MmaCtx *mma = nullptr;
-    if constexpr (MmaEnabled<T>::value) {
+    if constexpr (MMA) {
         if (L.mma_off >= 0 && clip) {
             uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
             mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
@@ -272,7 +279,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
         PHASE(1);
-        const int nw = shinv_block<T>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256),
+        const int nw = shinv_block<T, MMA>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256),
                                       (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
         PHASE(2);
@@ -327,7 +334,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 lin_zero<T>(Q, qlen);
             } else {
                 const int dlo = (h - 1) / 32;              // tensor-core form: E < B^(32 dlo + 1) <= B^h
-                int pl = try_mma_range<T>(mma, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
+                int pl = try_mma_range<T, MMA>(mma, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
                 if (pl >= 0) {
                     count(CNT_MMA_PRODUCTS);
                     lin_copy<T>(Q, qlen, PQ, pl, h - 32 * dlo);
@@ -344,7 +351,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             rlen = round_up(k + 3, TILE);
             int pl = 0;
             if (pq > 0) {
-                pl = try_mma_range<T>(mma, Vb, k + 1, Q, pq, 0, (rlen + 31) / 32, PQ, mq.HI, blk);
+                pl = try_mma_range<T, MMA>(mma, Vb, k + 1, Q, pq, 0, (rlen + 31) / 32, PQ, mq.HI, blk);
                 if (pl >= 0) {
                     count(CNT_MMA_PRODUCTS);
                     pl = min(rlen, pl);
@@ -387,7 +394,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         PHASE(7);
     }
     count_tiles(blk);
-    if constexpr (MmaEnabled<T>::value) {
+    if constexpr (MMA) {
         if (mma != nullptr) mma_fini<T>(mcx);
     }
 }
@@ -487,9 +494,8 @@ int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
                  cudaStream_t st, int clip, int sched)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    // (128-thread blocks: a latency-bound batch is faster on the IMAD path alone -- config 1 72 us against 100 us --
-    // and so are throughput batches of 2^15 bits, 7.07 M against 6.64 M div/s)
-    if (MmaEnabled<T>::value && clip && !(T <= 128 && (LAT || u_limbs < 1536)) && !getenv("MPDIV_NO_MMA"))
+    // (throughput batches of 2^15 bits are faster on the IMAD path alone: 7.07 M against 6.64 M div/s)
+    if (DivMma<T, LAT>::value && clip && !(T <= 128 && u_limbs < 1536) && !getenv("MPDIV_NO_MMA"))
         div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
