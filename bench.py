@@ -38,10 +38,11 @@ W_LIMB_PRODUCTS = {1024: 1898264, 2048: 7553425, 4096: 30136284, 8192: 120394683
 IMAD_PER_CLK_PER_SM = 64
 FLUSH_BYTES = 256 << 20   # > 126 MB of L2
 
-# DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_final.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 16292352 + 1147904, 3: 39562752 + 24485632, 4: 38811904 + 23737856}
+# DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_tensor_2p16.md)
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 24250368 + 7540480, 3: 39329536 + 24618240, 4: 38618880 + 23916800}
 # share of the division kernel in a device-resident step (the rest is the head kernel), same captures
-NCU_DIV_KERNEL_SHARE = {2: 400.2 / (400.2 + 43.6), 3: 798.4 / (798.4 + 43.6), 4: 1228.7 / (1228.7 + 40.3)}
+# (head kernel of configs 3 and 4 as captured in profiles/r1_final.md: it has not changed since)
+NCU_DIV_KERNEL_SHARE = {2: 284.7 / (284.7 + 42.3), 3: 679.7 / (679.7 + 43.6), 4: 849.8 / (849.8 + 40.3)}
 
 
 def parse_args():
@@ -403,7 +404,7 @@ def run_ours(args):
             "achieved": achieved / 1e9, "peak": peak_products / 1e9, "unit": "G limb-products/s",
             "frac": achieved / peak_products, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg),
             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture per launch "
-                              "(profiles/r1_final.md); algorithmic bytes per launch = %d" % (b * 4 * (2 * m + 2 * n)),
+                              "(profiles/r1_tensor_2p16.md); algorithmic bytes per launch = %d" % (b * 4 * (2 * m + 2 * n)),
             "peak_source": "measured in this run: mpdiv_imad_probe kind 0 (carry-chained IMAD.WIDE.U32 tile, no memory)",
             "nominal_imad32_peak": nominal_peak / 1e9,
             "measured_imad_lo32_peak": peaks["imad_lo32"] / 1e9,

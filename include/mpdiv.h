@@ -106,8 +106,9 @@ int mpmul_batch(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limbs,
  *   MPMUL_ENGINE_TENSOR  the product as an int8 tcgen05 GEMM: byte convolution with Toeplitz tiles generated
  *                        on the fly, accumulators in TMEM (csrc/mp_mma.cuh).  The north star allows tensor
  *                        cores only where measured faster: bench.py times both engines; mpdiv_batch uses this
- *                        engine for its large range products at 2^18 bits.  MPDIV_ERR_UNSUPPORTED when the
- *                        request needs more than 512 output blocks of 32 limbs or does not fit shared memory.
+ *                        engine for its large range products from 2^16 bits up (throughput batches).
+ *                        MPDIV_ERR_UNSUPPORTED when the request needs more than 512 output blocks of 32 limbs
+ *                        or does not fit shared memory.
  */
 #define MPMUL_ENGINE_IMAD 0
 #define MPMUL_ENGINE_TENSOR 1

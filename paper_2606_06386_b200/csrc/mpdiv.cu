@@ -11,7 +11,7 @@
 
 using namespace mpd;
 
-#define MPDIV_VERSION_STR "mpdiv 0.4 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
+#define MPDIV_VERSION_STR "mpdiv 0.5 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
 
 // ---------------------------------------------------------------------------------------
 // global <-> shared staging
