@@ -169,6 +169,18 @@ def measure_imad_peak(binding, iters: int = 4000):
     return out
 
 
+def measure_mma_issue(binding):
+    """Cycles per tcgen05.mma (M = 128, K = 32, u8) seen by one issuing warp and by two (mpdiv_mma_probe): the
+    tensor core needs N / 2; the rest is the issue path."""
+    out = {}
+    for n in (16, 64, 128):
+        one = binding.mma_probe(n, 1)
+        two = binding.mma_probe(n, 2)
+        out["N=%d" % n] = {"one_warp_cycles_per_mma": one[0], "two_warps_cycles_per_mma_together": max(two) / 2.0,
+                           "tensor_core_cycles_per_mma": n / 2.0}
+    return out
+
+
 def cpu_baseline(cfg: int, target_core_seconds: float = 16.0):
     """The oracle as it stands (Knuth D, one instance per call, batch split over host threads), timed on a
     bounded sample of the same workload: whole passes over the first instances of the batch until about
@@ -440,6 +452,7 @@ def run_ours(args):
         out["throughput_2^15_bits"] = {"batch": 32 * 148, "u_limbs": 1024, "v_limbs": 512, "div_ms": t15,
                                        "div_per_s": 32 * 148 / (t15 * 1e-3),
                                        "roofline_frac": 32 * 148 / (t15 * 1e-3) * W_LIMB_PRODUCTS[1024] / peak_products}
+        out["tensor_issue_probe"] = measure_mma_issue(binding)
         out["cpu_baseline"] = cpu_baseline(cfg)
         out["paper_context"] = "A100, 64-bit digits (PAPER.md:481-484): div/mul 6.77x/6.66x/6.94x/9.73x at 2^18..2^15 bits; model 5-7"
     print(json.dumps(out))

@@ -174,6 +174,16 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
                      mpdiv_stream_t stream);
 
 /*
+ * Tensor-core issue-rate probe (profiles/r1_tensor_2p16.md): one 128-thread block per SM in which
+ * `issuers` warps (1 or 2) each issue `iters` steps of four tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols,
+ * 16 <= n_cols <= 128, multiple of 16) into their own accumulator columns, the way the multiplier issues them.
+ * cycles (DEVICE pointer, 2 words): SM cycles block 0's warp w needed for its 4 * iters instructions, 0 if a
+ * bounded wait gave up.  The tensor core needs n_cols / 2 cycles per instruction; what a single warp measures
+ * above that is its own issue path.  Asynchronous on `stream`.
+ */
+int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream);
+
+/*
  * Debug counters accumulated by every mpdiv_batch / shinv_batch launch since the last reset
  * (device-side atomics on a library-owned 128-byte buffer; reading them synchronises `stream`):
  *   out[0] instances with exactly one delta = -1 correction (u < v*q0)

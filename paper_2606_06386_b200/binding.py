@@ -53,6 +53,8 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_batch_host.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP, sz, _VOIDP]
         L.mpdiv_imad_probe_threads.argtypes = []
         L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
+        L.mpdiv_mma_probe.argtypes = [i, i, i, _VOIDP, _VOIDP]
+        L.mpdiv_mma_probe.restype = i
         L.mpdiv_debug_counters.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), i, _VOIDP]
         L.mpdiv_seed_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP]
         L.mpdiv_batch_launches.argtypes = [i, i, i]
@@ -67,7 +69,7 @@ def lib() -> ctypes.CDLL:
 
 
 EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
-           "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe",
+           "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_mma_probe",
            "mpdiv_debug_counters", "mpdiv_seed_batch", "mpdiv_batch_launches", "mpdiv_version", "mpdiv_strerror")
 
 
@@ -227,6 +229,15 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
     _raise(lib().mpdiv_imad_probe(sink.data_ptr(), int(kind), int(iters), ctypes.byref(prod),
                                   _stream_ptr(stream)), "mpdiv_imad_probe")
     return int(prod.value), sink
+
+
+def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, stream=None):
+    """Cycles per tcgen05.mma (M = 128, K = 32, u8, N = n_cols) of each issuing warp of block 0; synchronises."""
+    out = torch.zeros(2, dtype=torch.int64, device="cuda")
+    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), out.data_ptr(), _stream_ptr(stream)),
+           "mpdiv_mma_probe")
+    torch.cuda.synchronize()
+    return [c / (4.0 * iters) for c in out.tolist()[:issuers]]
 
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",

@@ -321,6 +321,66 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
+// ---------------------------------------------------------------------------------------
+// tensor-core issue-rate probe (include/mpdiv.h: mpdiv_mma_probe)
+// ---------------------------------------------------------------------------------------
+// One block of 128 threads per SM; `issuers` warps (1 or 2) each issue `iters` steps of four
+// tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols, A in tensor memory, B = swizzled shared-memory rows) into
+// their own accumulator columns, in the warp form the multiplier uses (mp_mma.cuh: operand words in ordinary
+// registers, one lane elected around the four MMAs and the commit).  Operand contents are arbitrary; nothing
+// is read back.  cycles[warp] of block 0 = clock64 from the first issue to the completion barrier.
+constexpr int MMA_PROBE_ROWS = 272;
+__global__ void __launch_bounds__(128)
+mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
+{
+    extern __shared__ __align__(1024) uint8_t psm[];
+    uint8_t *brows = psm, *bars = psm + MMA_PROBE_ROWS * 128;
+    for (int i = threadIdx.x; i < MMA_PROBE_ROWS * 32; i += 128) reinterpret_cast<uint32_t *>(psm)[i] = (uint32_t)i * 2654435761u;
+    MmaCtx cx;
+    mma_init<128>(cx, brows, MMA_PROBE_ROWS, bars, 512);
+    if (threadIdx.x == 0) {
+        mbar_init(cx.bar + 136, 1);                      // completion barrier of the second issuer
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_async_smem();
+    __syncthreads();
+    const int warp = threadIdx.x >> 5;
+    if (warp < issuers) {
+        const long long t0 = clock64();
+        const uint32_t idesc0 = mma_idesc(n_cols);
+        for (int it = 0; it < iters; ++it) {
+            uint32_t d_tmem = cx.tmem_base + 128u * (uint32_t)warp, a_tmem = cx.tmem_base + 256u + 32u * (uint32_t)(it & 3);
+            uint32_t b_lo = mma_desc_lo(smem_u32(brows + (it & 7) * 128)), idesc = idesc0, ebar = cx.bar + 64 + 8 * warp;
+            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(ebar));
+            if (elect_one()) {
+                tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, 1u);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
+                tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
+                tc_commit(ebar);
+            }
+        }
+        if (elect_one()) tc_commit(cx.bar + 128 + 8 * warp);
+        __syncwarp();
+        const bool ok = mbar_wait(cx.bar + 128 + 8 * warp, 0);
+        const long long t1 = clock64();
+        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) cycles[warp] = ok ? (unsigned long long)(t1 - t0) : 0ull;
+    }
+    mma_fini<128>(cx);
+}
+
+int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream)
+{
+    if (!cycles || iters <= 0 || (issuers != 1 && issuers != 2) || n_cols < 16 || n_cols > 128 || (n_cols & 15))
+        return MPDIV_ERR_BAD_ARG;
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    const int bytes = MMA_PROBE_ROWS * 128 + 1024;
+    if (cudaFuncSetAttribute(mma_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess)
+        return MPDIV_ERR_CUDA;
+    mma_probe_kernel<<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
 const char *mpdiv_version(void) { return MPDIV_VERSION_STR; }
 
 const char *mpdiv_strerror(int code)

@@ -114,3 +114,18 @@ def test_prec_and_compare_with_power_of_B(an):
     for h in (0, 1, an // 2, an - 1):
         _, flag = run(binding.LINOP_ANY, a, a, h, an)
         assert [int(f) for f in flag] == [1 if x >= (1 << (32 * h)) else 0 for x in vals], h
+
+
+@pytest.mark.gpu
+def test_mma_probe_rates():
+    """mpdiv_mma_probe: every bounded wait completes, and the measured cycles per tcgen05.mma are never below the
+    tensor core's N / 2 (two issuing warps share one tensor core) nor absurdly above it."""
+    from paper_2606_06386_b200 import binding
+    for n in (16, 64, 128):
+        one = binding.mma_probe(n, 1, iters=500)
+        two = binding.mma_probe(n, 2, iters=500)
+        assert one[0] > 0 and min(two) > 0, "a bounded wait gave up"
+        assert one[0] >= n / 2.0 * 0.98 and max(two) / 2.0 >= n / 2.0 * 0.98
+        assert one[0] < 400 and max(two) < 800
+    with pytest.raises(binding.MpdivError):
+        binding.mma_probe(24, 1)
