@@ -268,7 +268,21 @@ def test_div_random_effective_precisions_large(variant):
     check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions 2048", variant)
 
 
-@pytest.mark.parametrize("M,count", [(4096, 240), (8192, 96)])
+def test_div_uses_tensor_engine_at_2_16_bits_in_throughput_batches_only():
+    """128-thread blocks: a throughput batch of config 2's shape runs its large range products on the tensor core
+    (warp 0 produces and issues, mp_mma.cuh); the latency kernel of a small batch is compiled without the engine.
+    Both must give the oracle's answer."""
+    u, v = inputs.config(2, batch=592)                  # more than two blocks per SM: throughput kernel
+    binding.debug_counters(reset=True)
+    check_div(u, v, "config 2 shape, throughput batch")
+    cnt = binding.debug_counters(reset=True)
+    assert cnt["mma_products"] >= 2 * 592 and cnt["mma_wait_failures"] == 0
+    check_div(u[:64], v[:64], "config 2 shape, latency batch")
+    cnt = binding.debug_counters(reset=True)
+    assert cnt["mma_products"] == 0
+
+
+@pytest.mark.parametrize("M,count", [(2048, 600), (4096, 240), (8192, 96)])
 def test_div_random_effective_precisions_tensor_sizes(M, count):
     """Random effective precisions at the strides whose kernels carry the tensor-core engine: every shape of
     range product (and every decision of mma_plan) occurs, including operands far from 32-limb multiples."""
