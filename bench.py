@@ -43,6 +43,9 @@ NCU_DRAM_BYTES_PER_LAUNCH = {2: 24250368 + 7540480, 3: 39329536 + 24618240, 4: 3
 # share of the division kernel in a device-resident step (the rest is the head kernel), same captures
 # (head kernel of configs 3 and 4 as captured in profiles/r1_final.md: it has not changed since)
 NCU_DIV_KERNEL_SHARE = {2: 284.7 / (284.7 + 42.3), 3: 679.7 / (679.7 + 43.6), 4: 849.8 / (849.8 + 40.3)}
+# pipe activity of the division kernel in the same captures, % of elapsed cycles:
+# (sm__pipe_tensor_cycles_active, sm__pipe_fmaheavy_cycles_active, smsp__issue_active)
+NCU_PIPES = {2: (13.75, 17.31, 44.75), 3: (18.91, 14.92, 37.62), 4: (25.86, 17.35, 34.65)}
 
 
 def parse_args():
@@ -408,6 +411,9 @@ def run_ours(args):
                              "both engines on the same products",
             "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
                                 "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
+            "ncu_pipes_pct": (dict(zip(("tensor", "fmaheavy", "issue_active"), NCU_PIPES[cfg]),
+                                   source="profiles/r1_tensor_2p16.md: neither pipe is the limit, the kernel is bound by "
+                                          "the latency of the phases inside a block") if cfg in NCU_PIPES else None),
             "bound": "alu", "kernel": "mpdiv_kernel",
             "kernels_per_step": binding.batch_launches(m, b),
             "kernel_share_of_step": NCU_DIV_KERNEL_SHARE.get(cfg) if binding.batch_launches(m, b) == 2 else 1.0,
