@@ -201,7 +201,9 @@ constexpr int CORR_MAX = 64;
 template <int T, bool LAT>
 struct DivMma { static constexpr bool value = MmaEnabled<T>::value && !(LAT && T <= 128); };
 
-template <int T, bool LAT>
+// MMA = this instantiation carries the engine (at most DivMma<T, LAT>; 128-thread throughput blocks also exist
+// without it, for the sizes that never use it: its mere presence costs 2^15-bit batches 4 %).
+template <int T, bool LAT, bool MMA>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l,
@@ -220,8 +222,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     mq.OV = mq.HI + L.p_words_q;
     mq.C3 = mq.OV + round_up(L.p_words_q / TILE, 4);
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
-    // the latency kernel of 128-thread blocks is compiled without the tensor-core engine (DivMma)
-    constexpr bool MMA = DivMma<T, LAT>::value;
+    static_assert(!MMA || DivMma<T, LAT>::value, "no tensor-core engine for this block size");
     MmaCtx mcx;
     MmaCtx *mma = nullptr;
     if constexpr (MMA) {
@@ -489,16 +490,14 @@ static cudaMemPool_t head_pool()
     return pools[dev];
 }
 
-template <int T, bool LAT>
-int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-                 cudaStream_t st, int clip, int sched)
+template <int T, bool LAT, bool MMA>
+int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+                 cudaStream_t st, int clip, int sched, bool tensor)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    // (throughput batches of 2^15 bits are faster on the IMAD path alone: 7.07 M against 6.64 M div/s)
-    if (DivMma<T, LAT>::value && clip && !(T <= 128 && u_limbs < 1536) && !getenv("MPDIV_NO_MMA"))
-        div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
+    if (MMA && tensor) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
     const size_t bytes = (size_t)L.total_words * 4;
-    int rc = set_smem(mpdiv_kernel<T, LAT>, bytes);
+    int rc = set_smem(mpdiv_kernel<T, LAT, MMA>, bytes);
     if (rc != MPDIV_OK) return rc;
     // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
     // iterate over in a stream-ordered workspace (mp_div.cuh "Head of Refine")
@@ -512,10 +511,24 @@ int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
             shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
         }
     }
-    mpdiv_kernel<T, LAT><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched), wmid);
+    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched), wmid);
     const bool ok = cudaGetLastError() == cudaSuccess;
     if (wmid) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+template <int T, bool LAT>
+int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+                 cudaStream_t st, int clip, int sched)
+{
+    // tensor-core range products: clipped variant only; 128-thread blocks from 2^16 bits up (throughput batches of
+    // 2^15 bits are faster on the IMAD path alone, 7.05 M against 6.64 M div/s, and run the instantiation without
+    // the engine)
+    const bool tensor = DivMma<T, LAT>::value && clip && !(T <= 128 && u_limbs < 1536) && !getenv("MPDIV_NO_MMA");
+    if constexpr (T == 128 && !LAT) {
+        if (!tensor) return launch_div_m<T, LAT, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, false);
+    }
+    return launch_div_m<T, LAT, DivMma<T, LAT>::value>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tensor);
 }
 
 // sched = the number of divisions that share the GPU with this launch (the batch itself, or the whole batch
