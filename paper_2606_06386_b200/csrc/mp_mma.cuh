@@ -37,7 +37,6 @@
 // Measured on B200 (mpmul_batch_ex, whole batches): 592 full 4096 x 4096-limb products in 0.245 ms = 4.1e13
 // limb products/s against 9.15e12 for the IMAD.WIDE roofline probe; 1184 x (2048 x 2048) in 0.226 ms.
 #pragma once
-#include <type_traits>
 #include "mp_block.cuh"
 
 namespace mpd {
@@ -341,42 +340,26 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     using Roles = MmaRoles<T>;
     constexpr int G = Roles::GROUPS;
     const uint32_t a_tmem0 = cx.tmem_base + (uint32_t)cx.acc_cols;
-    // MMAs k0 <= k < k1 of one step for the accumulator columns nc .. nc+255: D[:, nc..] += A_p x B_p, K = 128 as
-    // four instructions of K = 32.  WARP = true: called by a whole converged warp, one elected lane issues (the
-    // election sits directly around the straight-line tcgen05 code: with a loop inside the elected region ptxas
-    // falls back to its ELECT / BRA.U.ANY loop around every instruction); false: called by one thread.
-    // Only products wider than 256 output blocks come here; the common case is inlined in warp_issue.
-    auto issue_mmas = [&](int step, int s, int nc, int k0, int k1, auto warp_form) {
-        constexpr bool WARP = decltype(warp_form)::value;
+    // The four MMAs of one step for the accumulator columns nc .. nc+255 (products wider than 256 output blocks
+    // only; the common case is inlined in warp_issue): D[:, nc..] += A_p x B_p, K = 128 as four instructions of
+    // K = 32.  Called by a whole converged warp; one elected lane issues.  The election sits directly around the
+    // straight-line tcgen05 code: with a loop inside the elected region ptxas falls back to an ELECT / BRA.U.ANY
+    // loop around every instruction.
+    auto issue_mmas = [&](int step, int s, int nc) {
         const int p = pmin + step;
         uint32_t d_tmem = cx.tmem_base + (uint32_t)nc;
         uint32_t a_tmem = a_tmem0 + (uint32_t)(MMA_STAGE_COLS * s);
         uint32_t b_lo = mma_desc_lo(smem_u32(cx.brows + (dlo + nc - p - e0) * 128));   // + 2 per K slice of 32 bytes
         uint32_t idesc = mma_idesc(min(256, Nn - nc));
-        uint32_t acc0 = (step > 0 || k0 > 0) ? 1u : 0u;
-        uint32_t ak[4], bk[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { ak[k] = a_tmem + 8 * k; bk[k] = b_lo + 2 * k; }
-        if constexpr (WARP) {
-            // every lane computes the operand words; the empty asm keeps the arithmetic out of the elected branch
-            asm volatile("" : "+r"(d_tmem), "+r"(idesc), "+r"(acc0));
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (k >= k0 && k < k1) asm volatile("" : "+r"(ak[k]), "+r"(bk[k]));
+        uint32_t acc0 = step > 0 ? 1u : 0u;
+        // every lane computes the operand words; the empty asm keeps the arithmetic out of the elected branch
+        asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(acc0));
+        if (elect_one()) {
+            tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, acc0);
+            tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
+            tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
+            tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
         }
-        bool lead = true;
-        if constexpr (WARP) lead = elect_one();
-        if (lead) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (k >= k0 && k < k1) tc_mma_i8_ts_lo(d_tmem, ak[k], bk[k], idesc, k == k0 ? acc0 : 1u);
-        }
-    };
-    // the commit that frees the step's Toeplitz stage s
-    auto commit_stage = [&](int s, auto warp_form) {
-        bool lead = true;
-        if constexpr (decltype(warp_form)::value) lead = elect_one();
-        if (lead) tc_commit(cx.bar + 64 + 8 * s);
     };
     // One step issued by a whole converged warp: poll the tile's `full` barrier (stage s, parity par), then one
     // elected lane issues the MMAs and the commit.  b_lo = descriptor word of the row that column 0 reads at this
@@ -398,8 +381,8 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
                 tc_commit(ebar);
             }
         } else {
-            for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc, 0, 4, std::true_type{});
-            commit_stage(s, std::true_type{});
+            for (int nc = 0; nc < Nn; nc += 256) issue_mmas(step, s, nc);
+            if (elect_one()) tc_commit(cx.bar + 64 + 8 * s);      // frees the step's Toeplitz stage
         }
         return true;
     };
