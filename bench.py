@@ -38,14 +38,23 @@ W_LIMB_PRODUCTS = {1024: 1898264, 2048: 7553425, 4096: 30136284, 8192: 120394683
 IMAD_PER_CLK_PER_SM = 64
 FLUSH_BYTES = 256 << 20   # > 126 MB of L2
 
-# DRAM bytes per launch of the division kernel from the committed ncu captures (profiles/r1_tensor_2p16.md)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 24250368 + 7540480, 3: 39329536 + 24618240, 4: 38618880 + 23916800}
-# share of the division kernel in a device-resident step (the rest is the head kernel), same captures
-# (head kernel of configs 3 and 4 as captured in profiles/r1_final.md: it has not changed since)
-NCU_DIV_KERNEL_SHARE = {2: 284.7 / (284.7 + 42.3), 3: 679.7 / (679.7 + 43.6), 4: 849.8 / (849.8 + 40.3)}
-# pipe activity of the division kernel in the same captures, % of elapsed cycles:
-# (sm__pipe_tensor_cycles_active, sm__pipe_fmaheavy_cycles_active, smsp__issue_active)
-NCU_PIPES = {2: (13.75, 17.31, 44.75), 3: (18.91, 14.92, 37.62), 4: (25.86, 17.35, 34.65)}
+# ncu-derived figures (DRAM traffic per launch, kernel share of a step, pipe activity) are NOT measured by this
+# script: they are read from a committed summary that names the commit and the command it was captured with
+# (profiles/ncu_summary.json, written from the .ncu-rep files by hand-run ncu exports), or reported as null.
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "ncu_summary.json")
+
+
+def ncu_summary(cfg: int):
+    try:
+        with open(NCU_SUMMARY) as f:
+            doc = json.load(f)
+        row = doc.get("configs", {}).get(str(cfg))
+        if row is None:
+            return None
+        return dict(row, commit=doc.get("commit"), source="profiles/ncu_summary.json (captured at that commit; "
+                    "per-launch times under ncu are cold-cache and serialised: compare shares, not absolutes)")
+    except (OSError, ValueError):
+        return None
 
 
 def parse_args():
@@ -84,7 +93,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
@@ -172,6 +181,28 @@ def measure_imad_peak(binding, iters: int = 4000):
     return out
 
 
+def measure_tensor_peak(binding, iters: int = 20000):
+    """u8 x u8 multiply-accumulates per second of the tensor pipe, measured: two warps of one block per SM issue
+    tcgen05.mma.kind::i8 (M = 128, N = 128, K = 32) back to back into disjoint accumulators (mpdiv_mma_probe);
+    best of 5 launches timed with events.  Nominal: 8192 MAC per clock per SM."""
+    import torch
+
+    out = torch.zeros(2, dtype=torch.int64, device="cuda")
+    macs = binding.mma_probe_macs(128, 2, iters)
+    best = None
+    for _ in range(6):
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        binding.mma_probe_launch(128, 2, iters, out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None or ms < best else best
+    assert int(out.min().item()) > 0, "mpdiv_mma_probe: a bounded wait gave up"
+    return macs / (best * 1e-3)
+
+
 def measure_mma_issue(binding):
     """Cycles per tcgen05.mma (M = 128, K = 32, u8) seen by one issuing warp and by two (mpdiv_mma_probe): the
     tensor core needs N / 2; the rest is the issue path."""
@@ -216,74 +247,95 @@ def cpu_baseline(cfg: int, target_core_seconds: float = 16.0):
 # ----------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------
-def per_config_table(binding, flush, peak_products: float):
-    """divisions/s, shinv and multiplication times and the cost ratios of SURVEY.md G12 for configs 1-5
-    (25 timed runs each, the paper's count; median)."""
+MAC_PER_COLSTEP = 4 * 128 * 32      # one MMA step = 4 instructions of M = 128, K = 32 per accumulator column
+
+
+def executed_work(binding, du, dv, q, r, variant=None):
+    """What ONE launch really executes, counted by the kernels themselves (mpdiv_debug_counters): limb products on
+    the IMAD pipe (8x8 tiles x 64, tile padding included) and u8 x u8 multiply-accumulates on the tensor pipe
+    (MMA steps x accumulator columns x 16384, column padding included)."""
+    import torch
+
+    binding.debug_counters(reset=True)
+    binding.mpdiv_batch(du, dv, q, r, variant=variant)
+    torch.cuda.synchronize()
+    c = binding.debug_counters(reset=True)
+    return 64 * c["tiles"], MAC_PER_COLSTEP * c["mma_colsteps"], c
+
+
+def pipe_fractions(imad_products, tensor_macs, ms, peaks):
+    """Executed work / time / measured peak of each pipe, and which one is the (nearer) bound."""
+    t = ms * 1e-3
+    f_imad = imad_products / t / peaks["imad_wide_chain"]
+    f_tc = tensor_macs / t / peaks["tensor_u8_mac"]
+    return f_imad, f_tc, ("tensor" if f_tc >= f_imad else "alu")
+
+
+def config_row(binding, cfg, flush, peaks):
+    """divisions/s, both pipe fractions, the printed variant's work-conserving fraction and the cost ratios of
+    SURVEY.md G12 for one config (25 timed runs each, the paper's count PAPER.md:476; median)."""
     import torch
 
     from paper_2606_06386_b200 import inputs
 
-    table = {}
-    for cfg in (1, 2, 3, 4, 5):
-        b, m, n = inputs.CONFIG_SHAPES[cfg]
-        u, v = inputs.config(cfg)
-        du, dv = to_dev(u), to_dev(v)
-        q = torch.empty_like(du)
-        r = torch.empty_like(dv)
-        t_div = float(np.median(time_steps(lambda: binding.mpdiv_batch(du, dv, q, r), 25, 3, flush)))
-        t_div_printed = float(np.median(time_steps(
-            lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED), 25, 3, flush)))
-        executed = executed_products(binding, du, dv, q, r)
-        # R1 unit: M x M -> low M limbs (the paper's "full multiplication", M^2/2 limb products, PAPER.md:448)
-        a1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 0), b, m))
-        b1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 1), b, m))
-        c1 = torch.empty((b, m), dtype=torch.int32, device="cuda")
-        t_m1 = float(np.median(time_steps(lambda: binding.mpmul_batch(a1, b1, m, c1), 25, 3, flush)))
-        # R2 unit: n x n -> 2n limbs, the full product of two divisor-sized numbers (M^2/4 limb products)
-        nn = max(n if cfg != 5 else m // 2, 4)
-        a2 = a1[:, :nn].contiguous()
-        b2 = b1[:, :nn].contiguous()
-        c2 = torch.empty((b, 2 * nn), dtype=torch.int32, device="cuda")
-        t_m2 = float(np.median(time_steps(lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2), 25, 3, flush)))
-        # the same two products on the tensor-core engine (int8 tcgen05), where it fits
-        t_m1_tc = t_m2_tc = None
-        try:
-            t_m1_tc = float(np.median(time_steps(
-                lambda: binding.mpmul_batch(a1, b1, m, c1, engine=binding.ENGINE_TENSOR), 25, 3, flush)))
-        except binding.MpdivError:
-            pass
-        try:
-            t_m2_tc = float(np.median(time_steps(
-                lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2, engine=binding.ENGINE_TENSOR), 25, 3, flush)))
-        except binding.MpdivError:
-            pass
-        wl = (m + 1 + 3) // 4 * 4
-        w = torch.empty((b, wl), dtype=torch.int32, device="cuda")
-        t_sh = float(np.median(time_steps(lambda: binding.shinv_batch(dv, m, wl, w), 25, 3, flush)))
-        row = {
-            "batch": b, "u_limbs": m, "v_limbs": n,
-            "div_ms": t_div, "div_per_s": b / (t_div * 1e-3), "us_per_div_latency": t_div * 1e3 if cfg == 1 else None,
-            "mul_MxM_lowM_ms": t_m1, "mul_nxn_full_ms": t_m2, "shinv_ms": t_sh,
-            "R1_div_over_mul_MxM_lowM": t_div / t_m1, "R2_div_over_mul_nxn_full": t_div / t_m2,
-            "shinv_over_mul_MxM_lowM": t_sh / t_m1,
-            "mul_MxM_lowM_products_per_s": b * (m * (m + 1) / 2) / (t_m1 * 1e-3),
-            "mul_nxn_full_products_per_s": b * nn * nn / (t_m2 * 1e-3),
-            "hbm_GBps_div_io": b * 4 * (2 * m + 2 * n) / (t_div * 1e-3) / 1e9,
-            "mul_MxM_lowM_tensor_ms": t_m1_tc, "mul_nxn_full_tensor_ms": t_m2_tc,
-            "mul_nxn_full_tensor_products_per_s": (b * nn * nn / (t_m2_tc * 1e-3)) if t_m2_tc else None,
-            "tensor_over_imad_speedup_nxn_full": (t_m2 / t_m2_tc) if t_m2_tc else None,
-            "printed_variant_div_ms": t_div_printed, "printed_variant_div_per_s": b / (t_div_printed * 1e-3),
-            "printed_variant_R1": t_div_printed / t_m1,
-            "executed_limb_products_per_division": executed / b,
-            "pipe_frac_executed": executed / (t_div * 1e-3) / peak_products,
-        }
-        if cfg != 5:
-            row["W_limb_products"] = W_LIMB_PRODUCTS[m]
-            row["roofline_frac"] = row["div_per_s"] * W_LIMB_PRODUCTS[m] / peak_products
-            row["printed_variant_roofline_frac"] = row["printed_variant_div_per_s"] * W_LIMB_PRODUCTS[m] / peak_products
-        table["config%d" % cfg] = row
-        del du, dv, q, r, a1, b1, c1, a2, b2, c2, w
-    return table
+    b, m, n = inputs.CONFIG_SHAPES[cfg]
+    u, v = inputs.config(cfg)
+    du, dv = to_dev(u), to_dev(v)
+    q = torch.empty_like(du)
+    r = torch.empty_like(dv)
+    med = lambda fn: float(np.median(time_steps(fn, 25, 3, flush)))   # noqa: E731
+    t_div = med(lambda: binding.mpdiv_batch(du, dv, q, r))
+    t_div_printed = med(lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED))
+    ex_imad, ex_tc, _ = executed_work(binding, du, dv, q, r)
+    exp_imad, exp_tc, _ = executed_work(binding, du, dv, q, r, variant=binding.VARIANT_PRINTED)
+    f_imad, f_tc, bound = pipe_fractions(ex_imad, ex_tc, t_div, peaks)
+    # R1 unit: M x M -> low M limbs (the paper's "full multiplication", M^2/2 limb products, PAPER.md:448);
+    # R2 unit: n x n -> 2n limbs; each on both engines
+    a1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 0), b, m))
+    b1 = to_dev(inputs._uniform(inputs.rng_for(500 + cfg, 1), b, m))
+    c1 = torch.empty((b, m), dtype=torch.int32, device="cuda")
+    nn = max(n if cfg != 5 else m // 2, 4)
+    a2 = a1[:, :nn].contiguous()
+    b2 = b1[:, :nn].contiguous()
+    c2 = torch.empty((b, 2 * nn), dtype=torch.int32, device="cuda")
+    t_m1 = med(lambda: binding.mpmul_batch(a1, b1, m, c1))
+    t_m2 = med(lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2))
+    t_m1_tc = t_m2_tc = None
+    try:
+        t_m1_tc = med(lambda: binding.mpmul_batch(a1, b1, m, c1, engine=binding.ENGINE_TENSOR))
+        t_m2_tc = med(lambda: binding.mpmul_batch(a2, b2, 2 * nn, c2, engine=binding.ENGINE_TENSOR))
+    except binding.MpdivError:
+        pass
+    wl = (m + 1 + 3) // 4 * 4
+    w = torch.empty((b, wl), dtype=torch.int32, device="cuda")
+    t_sh = med(lambda: binding.shinv_batch(dv, m, wl, w))                                       # Theorem 2's value
+    t_sh_clip = med(lambda: binding.shinv_batch(dv, m, wl, w, variant=binding.VARIANT_CLIPPED))  # what Div runs
+    assert binding.status(reset=True) == 0, "mpdiv_status reported a fault during the per-config runs"
+    row = {
+        "batch": b, "u_limbs": m, "v_limbs": n, "bits": 32 * m,
+        "div_ms": t_div, "div_per_s": b / (t_div * 1e-3), "us_per_div_latency": t_div * 1e3 if b <= 148 else None,
+        "frac_imad_pipe": f_imad, "frac_tensor_pipe": f_tc, "bound": bound, "frac": max(f_imad, f_tc),
+        "executed_limb_products_per_div": ex_imad / b, "executed_tensor_macs_per_div": ex_tc / b,
+        "printed_div_per_s": b / (t_div_printed * 1e-3),
+        "frac_printed": exp_imad / (t_div_printed * 1e-3) / peaks["imad_wide_chain"],
+        "mul_MxM_lowM_ms": {"imad": t_m1, "tensor": t_m1_tc}, "mul_nxn_full_ms": {"imad": t_m2, "tensor": t_m2_tc},
+        "shinv_ms": {"printed": t_sh, "clipped": t_sh_clip},
+        # R1 = T(div) / T(M x M -> low M); the default division against BOTH multiplication engines, and the
+        # printed division against the IMAD engine (the paper-comparable pairing: same engine on both sides)
+        "R1": {"printed_div_over_imad_mul": t_div_printed / t_m1, "div_over_imad_mul": t_div / t_m1,
+               "div_over_tensor_mul": (t_div / t_m1_tc) if t_m1_tc else None},
+        "R2": {"printed_div_over_imad_mul": t_div_printed / t_m2, "div_over_imad_mul": t_div / t_m2,
+               "div_over_tensor_mul": (t_div / t_m2_tc) if t_m2_tc else None},
+        "shinv_over_mul_MxM_lowM": {"printed_over_imad": t_sh / t_m1,
+                                    "clipped_over_tensor": (t_sh_clip / t_m1_tc) if t_m1_tc else None},
+        "mul_imad_products_per_s": b * nn * nn / (t_m2 * 1e-3),
+        "mul_tensor_products_per_s": (b * nn * nn / (t_m2_tc * 1e-3)) if t_m2_tc else None,
+        "hbm_GBps_div_io": b * 4 * (2 * m + 2 * n) / (t_div * 1e-3) / 1e9,
+    }
+    if cfg != 5:
+        row["W_limb_products"] = W_LIMB_PRODUCTS[m]
+        row["speedup_vs_printed_work"] = row["div_per_s"] * W_LIMB_PRODUCTS[m] / peaks["imad_wide_chain"]
+    return row
 
 
 # The paper's own workload shape (PAPER.md:474): prec(u) = M - 2, prec(v) uniform in 2..M/2, with the
@@ -310,16 +362,6 @@ def paper_shape_table(binding, flush):
                     "paper's Table 1 (64-bit digits, other hardware): context only"}
         del du, dv, q, r
     return table
-
-
-def executed_products(binding, du, dv, q, r, variant=None) -> int:
-    """Limb products one launch really issues (8x8 tiles counted by the kernel x 64, tile padding included)."""
-    import torch
-
-    binding.debug_counters(reset=True)
-    binding.mpdiv_batch(du, dv, q, r, variant=variant)
-    torch.cuda.synchronize()
-    return 64 * binding.debug_counters(reset=True)["tiles"]
 
 
 def run_ours(args):
@@ -353,33 +395,34 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident throughput ------------------------------------------------------------
+    hu = torch.from_numpy(u.view(np.int32)).pin_memory()
+    hv = torch.from_numpy(v.view(np.int32)).pin_memory()
+    hq = torch.empty_like(hu).pin_memory()
+    hr = torch.empty_like(hv).pin_memory()
+    ws = torch.empty(binding.host_workspace_bytes(m, n, b), dtype=torch.uint8, device="cuda")
+    binding.status(reset=True)
+
+    # ---- device-resident throughput, then end to end (host buffers through mpdiv_batch_host: H2D + division +
+    # D2H inside the timing); the clock sampler runs over both timed regions
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
     t0 = time.time()
     ms = time_steps(lambda: binding.mpdiv_batch(du, dv, q, r), args.steps, args.warmup, flush)
     barrier()
+    ms_e = time_steps(lambda: binding.mpdiv_batch_host(hu, hv, hq, hr, ws), args.steps, args.warmup, flush)
+    barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
     total_ms = shard.max_over_ranks(float(sum(ms)), device="cuda")
     ms_per_step = total_ms / args.steps
     value = shard.aggregate_rate(b, world, ms_per_step)
-
-    # ---- end to end: host buffers through mpdiv_batch_host (H2D + division + D2H inside the timing) ----
-    hu = torch.from_numpy(u.view(np.int32)).pin_memory()
-    hv = torch.from_numpy(v.view(np.int32)).pin_memory()
-    hq = torch.empty_like(hu).pin_memory()
-    hr = torch.empty_like(hv).pin_memory()
-    ws = torch.empty(binding.host_workspace_bytes(m, n, b), dtype=torch.uint8, device="cuda")
-    barrier()
-    ms_e = time_steps(lambda: binding.mpdiv_batch_host(hu, hv, hq, hr, ws), args.steps, args.warmup, flush)
-    barrier()
     e_total = shard.max_over_ranks(float(sum(ms_e)), device="cuda")
     e2e_value = shard.aggregate_rate(b, world, e_total / args.steps)
     io_bytes = b * 4 * (m + n)
     # the device-timed result and the host round trip must agree bit for bit (cheap self-consistency)
     same = bool((hq.cuda() == q).all().item() and (hr.cuda() == r).all().item())
+    status = binding.status(reset=True)
 
     if world > 1:
         dist.barrier()
@@ -387,49 +430,50 @@ def run_ours(args):
     if rank != 0:
         return
 
-    # ---- roofline of the dominant kernel (a step = the head kernel + the division kernel, timed together) ---
+    # ---- roofline: what the timed step EXECUTED on each pipe, against peaks measured in this run -----------
     peaks = measure_imad_peak(binding)
+    peaks["tensor_u8_mac"] = measure_tensor_peak(binding)
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
-    nominal_peak = sm_count * IMAD_PER_CLK_PER_SM * 1965e6          # 32-bit IMAD/s at the max SM clock
-    peak_products = peaks["imad_wide_chain"]
     kernel_ms = float(np.mean(ms))
-    roofline = None
+    ex_imad, ex_tc, counters = executed_work(binding, du, dv, q, r)
+    f_imad, f_tc, bound = pipe_fractions(ex_imad, ex_tc, kernel_ms, peaks)
+    launches = binding.batch_launches(m, b)
+    ncu = ncu_summary(cfg)
+    if bound == "tensor":
+        achieved, peak, unit = ex_tc / (kernel_ms * 1e-3) / 1e12, peaks["tensor_u8_mac"] / 1e12, "T u8-MAC/s"
+    else:
+        achieved, peak, unit = ex_imad / (kernel_ms * 1e-3) / 1e9, peaks["imad_wide_chain"] / 1e9, "G limb-products/s"
+    roofline = {
+        "bound": bound, "achieved": achieved, "peak": peak, "unit": unit, "frac": max(f_imad, f_tc),
+        "definition": "frac = max over the two arithmetic pipes of (work the timed step EXECUTED on that pipe, counted "
+                      "by the kernels) / (step time) / (that pipe's peak measured in this run); recompute it from the "
+                      "executed_* and peak_* fields of this dict and ms_per_step",
+        "frac_imad_pipe": f_imad, "frac_tensor_pipe": f_tc,
+        "executed_limb_products_per_launch": ex_imad, "executed_tensor_macs_per_launch": ex_tc,
+        "peak_imad_limb_products_per_s": peaks["imad_wide_chain"], "peak_tensor_u8_macs_per_s": peaks["tensor_u8_mac"],
+        "peak_source": "measured in this run: mpdiv_imad_probe kind 0 (carry-chained IMAD.WIDE.U32 tile, no memory; "
+                       "nominal 32/clk/SM) and mpdiv_mma_probe (tcgen05.mma.kind::i8 M=128 N=128 K=32 from two warps, "
+                       "events; nominal 8192 MAC/clk/SM)",
+        "nominal_peaks": {"imad_limb_products_per_s": sm_count * 32 * 1965e6, "tensor_u8_macs_per_s": sm_count * 8192 * 1965e6,
+                          "imad_lo32_per_s_measured": peaks["imad_lo32"]},
+        "kernel": "mpdiv_kernel", "kernels_per_step": launches,
+        "timed_region": "CUDA events around the whole step on the launch stream (shinv_head_kernel + mpdiv_kernel when "
+                        "kernels_per_step = 2): achieved and frac charge the head kernel's time to the step",
+        "traffic": (ncu or {}).get("dram_bytes_per_launch"), "ncu": ncu,
+        "algorithmic_bytes_per_launch": b * 4 * (2 * m + 2 * n),
+        "hbm_GBps_io": b * 4 * (2 * m + 2 * n) / (kernel_ms * 1e-3) / 1e9,
+    }
     if cfg != 5:
-        achieved = b * W_LIMB_PRODUCTS[m] / (kernel_ms * 1e-3)
-        executed = executed_products(binding, du, dv, q, r)
-        ms_printed = float(np.mean(time_steps(
-            lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED), args.steps, args.warmup, flush)))
-        roofline = {
-            "note": "achieved = W(M) x batch / t with W(M) the limb products of the method AS PRINTED (SURVEY 8(d)); the "
-                    "default (clipped) variant skips the low part of w*x and u*shinv, the low and high parts of v'w and the "
-                    "high part of v*q (PAPER.md:507, :542), so frac may exceed 1; pipe_frac counts the limb products that "
-                    "really ran on the IMAD pipe (the products that ran on the tensor cores are not in it)",
-            "executed_limb_products_per_launch": executed,
-            "pipe_frac": executed / (kernel_ms * 1e-3) / peak_products,
-            "tensor_engine": "range products with enough work (u*shinv, v*q and the last Refine steps) run as int8 "
-                             "tcgen05 GEMMs (csrc/mp_mma.cuh) in throughput batches from 2^16 bits up; per_config times "
-                             "both engines on the same products",
-            "printed_variant": {"ms": ms_printed, "divisions_per_s": b / (ms_printed * 1e-3),
-                                "frac": b * W_LIMB_PRODUCTS[m] / (ms_printed * 1e-3) / peak_products},
-            "ncu_pipes_pct": (dict(zip(("tensor", "fmaheavy", "issue_active"), NCU_PIPES[cfg]),
-                                   source="profiles/r1_tensor_2p16.md: neither pipe is the limit, the kernel is bound by "
-                                          "the latency of the phases inside a block") if cfg in NCU_PIPES else None),
-            "bound": "alu", "kernel": "mpdiv_kernel",
-            "kernels_per_step": binding.batch_launches(m, b),
-            "kernel_share_of_step": NCU_DIV_KERNEL_SHARE.get(cfg) if binding.batch_launches(m, b) == 2 else 1.0,
-            "timed_region": "CUDA events around the whole step (shinv_head_kernel + mpdiv_kernel on the launch stream): "
-                            "achieved and frac are per step, i.e. they charge the head kernel's time to the division",
-            "achieved": achieved / 1e9, "peak": peak_products / 1e9, "unit": "G limb-products/s",
-            "frac": achieved / peak_products, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg),
-            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture per launch "
-                              "(profiles/r1_tensor_2p16.md); algorithmic bytes per launch = %d" % (b * 4 * (2 * m + 2 * n)),
-            "peak_source": "measured in this run: mpdiv_imad_probe kind 0 (carry-chained IMAD.WIDE.U32 tile, no memory)",
-            "nominal_imad32_peak": nominal_peak / 1e9,
-            "measured_imad_lo32_peak": peaks["imad_lo32"] / 1e9,
-            "frac_of_nominal_imad32": achieved / nominal_peak,
-            "work_per_division": W_LIMB_PRODUCTS[m],
-            "hbm_GBps_io": b * 4 * (2 * m + 2 * n) / (kernel_ms * 1e-3) / 1e9,
-        }
+        roofline["work_per_division_as_printed"] = W_LIMB_PRODUCTS[m]
+        roofline["speedup_vs_printed_work"] = b * W_LIMB_PRODUCTS[m] / (kernel_ms * 1e-3) / peaks["imad_wide_chain"]
+        roofline["speedup_vs_printed_work_note"] = (
+            "divisions/s x W(M) / IMAD peak, W(M) = limb products of the method AS PRINTED (SURVEY 8(d)): how much "
+            "faster than an IMAD-roofline implementation of the printed algorithm; NOT a utilisation (the default "
+            "variant clips products, PAPER.md:507, :542, and runs the large ones on the tensor core)")
+    if not args.brief:
+        # one compact row per config INSIDE the roofline dict: div/s, both pipe fractions, the printed variant's
+        # work-conserving fraction, R1 against both multiplication engines
+        roofline["per_config"] = {"config%d" % c: config_row(binding, c, flush, peaks) for c in (1, 2, 3, 4, 5)}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -440,14 +484,16 @@ def run_ours(args):
                    "timing": "CUDA events per step on the launch stream, summed; max over ranks"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                 "api": "mpdiv_batch_host (pinned host buffers)", "matches_device_run": same},
-        "gpu_launches": args.steps * binding.batch_launches(m, b),
+        "gpu_launches": args.steps * launches,
         "clocks": clocks,
         "roofline": roofline,
+        "mpdiv_status": status,
         "step_ms_min_median_max": [float(np.min(ms)), float(np.median(ms)), float(np.max(ms))],
+        "counters_one_step": {k: counters[k] for k in ("tiles", "mma_colsteps", "mma_products", "clipped_steps",
+                                                       "cluster_divs", "delta_pos", "delta_neg")},
         "version": binding.version(),
     }
     if not args.brief:
-        out["per_config"] = per_config_table(binding, flush, peak_products)
         out["paper_shape"] = paper_shape_table(binding, flush)
         # config 1 has 32 instances (latency bound on 148 SMs); the same shape with 32 x 148 instances gives the
         # THROUGHPUT point of the metric at 2^15 bits
@@ -455,9 +501,12 @@ def run_ours(args):
         d15u, d15v = to_dev(u15), to_dev(v15)
         q15, r15 = torch.empty_like(d15u), torch.empty_like(d15v)
         t15 = float(np.median(time_steps(lambda: binding.mpdiv_batch(d15u, d15v, q15, r15), 25, 3, flush)))
+        e15, c15, _ = executed_work(binding, d15u, d15v, q15, r15)
+        f15 = pipe_fractions(e15, c15, t15, peaks)
         out["throughput_2^15_bits"] = {"batch": 32 * 148, "u_limbs": 1024, "v_limbs": 512, "div_ms": t15,
-                                       "div_per_s": 32 * 148 / (t15 * 1e-3),
-                                       "roofline_frac": 32 * 148 / (t15 * 1e-3) * W_LIMB_PRODUCTS[1024] / peak_products}
+                                       "div_per_s": 32 * 148 / (t15 * 1e-3), "frac_imad_pipe": f15[0],
+                                       "frac_tensor_pipe": f15[1],
+                                       "speedup_vs_printed_work": 32 * 148 / (t15 * 1e-3) * W_LIMB_PRODUCTS[1024] / peaks["imad_wide_chain"]}
         out["tensor_issue_probe"] = measure_mma_issue(binding)
         out["cpu_baseline"] = cpu_baseline(cfg)
         out["paper_context"] = "A100, 64-bit digits (PAPER.md:481-484): div/mul 6.77x/6.66x/6.94x/9.73x at 2^18..2^15 bits; model 5-7"
@@ -510,6 +559,12 @@ def run_reference(args):
 
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as plain `python bench.py --gpus N`: launch the N ranks ourselves (one process per GPU, NCCL
+        # used for the barrier and the max-over-ranks time only) and pass their exit code on
+        from paper_2606_06386_b200 import shard
+
+        raise SystemExit(subprocess.call(shard.torchrun_argv(args.gpus, os.path.abspath(__file__), sys.argv[1:])))
     if args.impl == "reference":
         run_reference(args)
     else:

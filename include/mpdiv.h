@@ -15,11 +15,17 @@
  *     precision themselves ("Prec").
  *   - Pointers of the *_batch functions are DEVICE pointers owned by the caller (PyTorch allocates
  *     them); they must be 16-byte aligned and every stride must be a multiple of 4 limbs.
- *     Outputs must not overlap inputs.  The library allocates no persistent memory, never frees
- *     caller memory and never synchronises the stream: work is enqueued on `stream` and the call
- *     returns.  The first call of each kernel sets its shared-memory attribute (host side only).
+ *     Outputs must not overlap inputs.  The library never frees caller memory and the *_batch calls
+ *     never synchronise the stream: work is enqueued on `stream` and the call returns.  Library-owned
+ *     state, all per device, created on first use and never destroyed: the shared-memory attribute of each
+ *     kernel, a memory pool for the stream-ordered workspace of mpdiv_batch (see there), the helper
+ *     streams and events of mpdiv_batch_host, and three small device words (counters, status).
  *   - Return value: MPDIV_OK, or an error code; nothing is enqueued when an error is returned.
  *     No exception crosses the ABI.  mpdiv_strerror() gives a text for a code.
+ *   - Conditions a kernel can only find while it runs (a tensor-core pipeline wait that gave up, a
+ *     correction loop that hit its bound, v = 0) do not change the return value of the asynchronous
+ *     call; they set sticky bits of a device status word that mpdiv_status() reads.  A caller that
+ *     needs certainty polls it once per batch (tests do so after every batch; it must read 0).
  *   - Supported sizes: strides up to MPDIV_MAX_LIMBS limbs (2^18 bits, the paper's range,
  *     PAPER.md:194); any effective precision inside the stride, including 0.
  */
@@ -32,15 +38,6 @@
 #ifdef __cplusplus
 extern "C" {
 #endif
-
-/*
- * Tuning switches (environment, read at every launch; for A/B measurements and the tests, not for production):
- *   MPDIV_NO_SEED=1   Refine starts at l = 2 as printed instead of the 17-digit seed (clipped variant)
- *   MPDIV_NO_HEAD=1   the head of Refine stays inside the division kernel (see mpdiv_batch_launches)
- *   MPDIV_NO_MMA=1    every product of the division runs on the IMAD engine (no tcgen05 range products)
- *   MPDIV_THREADS=n   block size override (64, 128, 256, 512)
- * None of them changes a result: q and r are exact either way.
- */
 
 /* binary-compatible with cudaStream_t (0 / NULL = the legacy default stream) */
 typedef struct CUstream_st *mpdiv_stream_t;
@@ -57,10 +54,11 @@ enum {
 /*
  * Division, Alg. 3: for each i < batch
  *     q_i = floor(u_i / v_i),   r_i = u_i - q_i * v_i        (u = q*v + r, 0 <= r < v)
- *   u : batch x u_limbs (device, read)      v : batch x v_limbs (device, read), v_limbs <= u_limbs
+ *   u : batch x u_limbs (device, read)      v : batch x v_limbs (device, read)
  *   q : batch x u_limbs (device, written)   r : batch x v_limbs (device, written)
  * q has stride u_limbs because the quotient of an M-limb by an n-limb number can need M-n+1
- * limbs, and up to M when the divisor is short; both outputs are zero padded.
+ * limbs, and up to M when the divisor is short; both outputs are zero padded.  v_limbs may exceed
+ * u_limbs (an instance whose divisor is really longer than its dividend gives q = 0, r = u).
  * v_i = 0 (undefined in the paper) does not trap: q_i is set to all ones, r_i to the
  * low v_limbs limbs of u_i, and the instance is counted in mpdiv_debug_counters.
  * Launches: one kernel, one division per thread block; a throughput batch of the clipped variant
@@ -81,13 +79,28 @@ int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
  *                          computes only the limb range the step keeps (top of w*x and u*shinv, middle
  *                          of v'w, bottom of v*q); the +-1 correction of Alg. 3 becomes two bounded
  *                          loops.  About 0.4 M^2 instead of 1.8 M^2 limb products per division.
- * mpdiv_batch / shinv_batch use MPDIV_VARIANT_DEFAULT.
+ * mpdiv_batch uses MPDIV_VARIANT_DEFAULT; shinv_batch returns Theorem 2's value and uses MPDIV_VARIANT_PRINTED.
+ *
+ * `flags` of the *_ex calls = a variant, optionally OR-ed with tuning switches (for A/B measurements and the
+ * tests; none of them changes a result, q and r are exact either way):
+ *   MPDIV_FLAG_NO_SEED     Refine starts at l = 2 as printed instead of the 17-digit seed (clipped variant)
+ *   MPDIV_FLAG_NO_HEAD     the head of Refine stays inside the division kernel (see mpdiv_batch_launches)
+ *   MPDIV_FLAG_NO_MMA      every product of the division runs on the IMAD engine (no tcgen05 range products)
+ *   MPDIV_FLAG_NO_CLUSTER  a small batch keeps one block per division (no thread-block cluster per division)
+ *   MPDIV_FLAG_THREADS(n)  block size override, n in {64, 128, 256, 512}
  */
 #define MPDIV_VARIANT_PRINTED 0
 #define MPDIV_VARIANT_CLIPPED 1
 #define MPDIV_VARIANT_DEFAULT MPDIV_VARIANT_CLIPPED
+#define MPDIV_VARIANT_MASK 0x0f
+#define MPDIV_FLAG_NO_SEED 0x10
+#define MPDIV_FLAG_NO_HEAD 0x20
+#define MPDIV_FLAG_NO_MMA 0x40
+#define MPDIV_FLAG_NO_CLUSTER 0x80
+#define MPDIV_FLAG_THREADS(n) ((n) == 64 ? 0x100 : (n) == 128 ? 0x200 : (n) == 256 ? 0x300 : (n) == 512 ? 0x400 : 0)
+#define MPDIV_FLAG_THREADS_MASK 0x700
 int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
-                   uint32_t *q, uint32_t *r, int batch, int variant, mpdiv_stream_t stream);
+                   uint32_t *q, uint32_t *r, int batch, int flags, mpdiv_stream_t stream);
 
 /*
  * Multiplication, the unit of the paper's cost model (PAPER.md:105-106 MULT / MULTMOD, :166, :186):
@@ -118,16 +131,21 @@ int mpmul_batch_ex(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limb
 /*
  * Whole shifted inverse as the division uses it, Alg. 1-2 and Theorem 2
  * (PAPER.md:160):   w_i = floor(B^h / v_i) + lambda_i,  lambda_i in {0, 1}
- * (lambda in {-1, 0, 1} for the clipped variant)
- * i.e. the UNCORRECTED Newton result, so that its time is the "2..4 multiplications" of the cost
- * model.   v : batch x v_limbs (device, read);  w : batch x w_limbs (device, written),
- * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_LIMBS.  v_i = 0 gives w_i = all ones (counted as an error).
+ * i.e. the UNCORRECTED Newton result of the algorithm as printed (MPDIV_VARIANT_PRINTED), so that its time
+ * is the "2..4 multiplications" of the cost model.
+ *   v : batch x v_limbs (device, read);  w : batch x w_limbs (device, written),
+ * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_LIMBS.  v_i = 0 gives w_i = all ones (status bit MPDIV_STATUS_V_ZERO).
  */
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
                 int batch, mpdiv_stream_t stream);
-/* Same with an explicit variant; the clipped variant returns floor(B^h / v) + lambda, lambda in {-1, 0, 1}. */
+/*
+ * Same with explicit flags (variant | tuning switches, see mpdiv_batch_ex).  MPDIV_VARIANT_CLIPPED is the
+ * shifted inverse as the default division computes it (clipped products, "+1" loop, 17-digit seed): it
+ * returns floor(B^h / v) + lambda with lambda in {-1, 0, 1}, one unit wider than Theorem 2; Div's bounded
+ * correction loops absorb it.
+ */
 int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
-                   int batch, int variant, mpdiv_stream_t stream);
+                   int batch, int flags, mpdiv_stream_t stream);
 
 /*
  * The linear-cost building blocks of the method on their own (PAPER.md 3.2-3.3), exported so that they can
@@ -155,7 +173,9 @@ int mplinop_batch(int op, const uint32_t *a, int a_limbs, const uint32_t *b, int
  * chunks share the SMs as the blocks of one launch would (six library-owned helper streams, created on
  * first use, never destroyed).  Everything is ordered after the work already enqueued on `stream`, and `stream`
  * completes only after the last D2H copy: the caller synchronises `stream` and reads q, r.
- * Reuse of the same events makes concurrent calls from several host threads unsupported.
+ * The helper streams and events belong to the current device; calls from several host threads are serialised
+ * by a lock around the enqueue.  When an error is returned part of the batch may have been enqueued: the call
+ * waits for that work before it returns, so the buffers are free again.
  */
 size_t mpdiv_host_workspace_bytes(int u_limbs, int v_limbs, int batch);
 int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host, int v_limbs,
@@ -174,18 +194,39 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
                      mpdiv_stream_t stream);
 
 /*
- * Tensor-core issue-rate probe (profiles/r1_tensor_2p16.md): one 128-thread block per SM in which
+ * Tensor-core issue-rate probe and int8 roofline probe: one 128-thread block per SM in which
  * `issuers` warps (1 or 2) each issue `iters` steps of four tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols,
  * 16 <= n_cols <= 128, multiple of 16) into their own accumulator columns, the way the multiplier issues them.
  * cycles (DEVICE pointer, 2 words): SM cycles block 0's warp w needed for its 4 * iters instructions, 0 if a
  * bounded wait gave up.  The tensor core needs n_cols / 2 cycles per instruction; what a single warp measures
- * above that is its own issue path.  Asynchronous on `stream`.
+ * above that is its own issue path.  One launch executes  SMs x issuers x iters x 4 x 128 x n_cols x 32
+ * u8 x u8 multiply-accumulates (mpdiv_mma_probe_macs); timed with events at n_cols = 128 and two issuers it
+ * gives the measured peak of the tensor pipe for this data type.  Asynchronous on `stream`.
  */
+unsigned long long mpdiv_mma_probe_macs(int n_cols, int issuers, int iters);
 int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream);
 
 /*
+ * Status word of the current device: sticky bits set by the kernels since the last reset.  Synchronises
+ * `stream`, stores the bits in *flags, clears them when `reset` is non-zero.  0 = every result delivered so
+ * far is exact.
+ *   MPDIV_STATUS_MMA_WAIT    a bounded wait of the tensor-core pipeline gave up; the block recomputed that
+ *                            product on the IMAD engine and stopped using the tensor core (results are still
+ *                            exact, the bit reports a protocol or scheduling fault)
+ *   MPDIV_STATUS_CORR_BOUND  a correction loop of Div hit its bound of 64 steps: that q, r is NOT exact
+ *   MPDIV_STATUS_REM_RANGE   clipped variant: the remainder estimate u - v*q0' left the range the
+ *                            mod-B^(k+3) arithmetic assumes (its top limb is neither 0 nor all ones): NOT exact
+ *   MPDIV_STATUS_V_ZERO      a divisor was zero (undefined): q = all ones, r = low limbs of u
+ */
+#define MPDIV_STATUS_MMA_WAIT 1u
+#define MPDIV_STATUS_CORR_BOUND 2u
+#define MPDIV_STATUS_REM_RANGE 4u
+#define MPDIV_STATUS_V_ZERO 8u
+int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset);
+
+/*
  * Debug counters accumulated by every mpdiv_batch / shinv_batch launch since the last reset
- * (device-side atomics on a library-owned 128-byte buffer; reading them synchronises `stream`):
+ * (a few device-side atomics per division on a library-owned buffer; reading them synchronises `stream`):
  *   out[0] instances with exactly one delta = -1 correction (u < v*q0)
  *   out[1] instances with exactly one delta = +1 correction
  *   out[2] instances needing more than one +1 step (printed variant: outside Theorem 2, expected 0;
@@ -200,8 +241,12 @@ int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycl
  *          pipeline waits that gave up (expected 0)
  *   out[14] add-back steps of the seed's long division (Knuth D6)      out[15] Shinv calls that started
  *          Refine from the 17-digit seed (mpdiv_seed_batch)
+ *   out[16] tensor-core work: sum over range products of (MMA steps x accumulator columns); x 16384 = the
+ *          u8 x u8 multiply-accumulates the tensor pipe executed (4 instructions of M = 128, K = 32 per step)
+ *   out[17] divisions that ran on a thread-block cluster      out[18..23] reserved (0)
  */
-int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream);
+#define MPDIV_NUM_COUNTERS 24
+int mpdiv_debug_counters(unsigned long long out[MPDIV_NUM_COUNTERS], int reset, mpdiv_stream_t stream);
 
 /*
  * The seed of Refine (clipped variant, csrc/mp_div.cuh warp_seed): for each divisor v >= B,
@@ -220,7 +265,7 @@ int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpd
  * and the Refine iterations up to l = 129 then run one warp per division ahead of the division kernel and
  * hand their iterate over in a stream-ordered workspace from a library-owned memory pool).  0 on bad arguments.
  */
-int mpdiv_batch_launches(int u_limbs, int batch, int variant);
+int mpdiv_batch_launches(int u_limbs, int batch, int flags);
 
 /* "mpdiv <version> sm_100a ..." */
 const char *mpdiv_version(void);

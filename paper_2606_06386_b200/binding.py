@@ -20,6 +20,16 @@ _VOIDP = ctypes.c_void_p
 OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
 VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
 VARIANT_DEFAULT = VARIANT_CLIPPED
+# tuning switches OR-ed into the `flags` of the *_ex calls (include/mpdiv.h)
+FLAG_NO_SEED, FLAG_NO_HEAD, FLAG_NO_MMA, FLAG_NO_CLUSTER = 0x10, 0x20, 0x40, 0x80
+STATUS_MMA_WAIT, STATUS_CORR_BOUND, STATUS_REM_RANGE, STATUS_V_ZERO = 1, 2, 4, 8
+NUM_COUNTERS = 24
+
+
+def flag_threads(n: int) -> int:
+    """MPDIV_FLAG_THREADS(n): block size override."""
+    return {64: 0x100, 128: 0x200, 256: 0x300, 512: 0x400}[int(n)]
+
 ENGINE_IMAD, ENGINE_TENSOR = 0, 1
 LINOP_ADD, LINOP_SUB, LINOP_NEG, LINOP_SHIFT, LINOP_PREC, LINOP_ANY = range(6)
 MAX_LIMBS = 8192
@@ -55,6 +65,10 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
         L.mpdiv_mma_probe.argtypes = [i, i, i, _VOIDP, _VOIDP]
         L.mpdiv_mma_probe.restype = i
+        L.mpdiv_mma_probe_macs.argtypes = [i, i, i]
+        L.mpdiv_mma_probe_macs.restype = ctypes.c_ulonglong
+        L.mpdiv_status.argtypes = [_VOIDP, ctypes.POINTER(ctypes.c_uint), i]
+        L.mpdiv_status.restype = i
         L.mpdiv_debug_counters.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), i, _VOIDP]
         L.mpdiv_seed_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP]
         L.mpdiv_batch_launches.argtypes = [i, i, i]
@@ -69,8 +83,8 @@ def lib() -> ctypes.CDLL:
 
 
 EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
-           "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_mma_probe",
-           "mpdiv_debug_counters", "mpdiv_seed_batch", "mpdiv_batch_launches", "mpdiv_version", "mpdiv_strerror")
+           "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_mma_probe", "mpdiv_mma_probe_macs",
+           "mpdiv_debug_counters", "mpdiv_status", "mpdiv_seed_batch", "mpdiv_batch_launches", "mpdiv_version", "mpdiv_strerror")
 
 
 def version() -> str:
@@ -103,7 +117,8 @@ def _raise(code: int, what: str):
 def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
                 r: torch.Tensor | None = None, stream=None, variant: int | None = None):
     """q = floor(u / v), r = u - q*v per row.  q has u's shape, r has v's shape.
-    variant: None -> mpdiv_batch (the library default), else mpdiv_batch_ex with that variant."""
+    variant: None -> mpdiv_batch (the library default), else mpdiv_batch_ex with these flags
+    (a VARIANT_* value, optionally OR-ed with FLAG_* tuning switches)."""
     _check_dev(u, "u")
     _check_dev(v, "v")
     batch, ul = u.shape
@@ -161,7 +176,9 @@ def mplinop_batch(op: int, a: torch.Tensor, b: torch.Tensor, shift: int, out_lim
 
 def shinv_batch(v: torch.Tensor, h: int, w_limbs: int, w: torch.Tensor | None = None, stream=None,
                 variant: int | None = None):
-    """w = floor(B^h / v) + lambda, lambda in {0, 1}, per row (the uncorrected Newton result)."""
+    """w = floor(B^h / v) + lambda per row (the uncorrected Newton result).  variant None -> shinv_batch: the
+    algorithm as printed, lambda in {0, 1} (Theorem 2); else shinv_batch_ex with these flags (VARIANT_CLIPPED:
+    lambda in {-1, 0, 1})."""
     _check_dev(v, "v")
     batch = v.shape[0]
     if w is None:
@@ -231,6 +248,12 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
     return int(prod.value), sink
 
 
+def mma_probe_launch(n_cols: int, issuers: int, iters: int, out: torch.Tensor, stream=None):
+    """Enqueue one probe launch (no synchronisation): for timing with events."""
+    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), out.data_ptr(), _stream_ptr(stream)),
+           "mpdiv_mma_probe")
+
+
 def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, stream=None):
     """Cycles per tcgen05.mma (M = 128, K = 32, u8, N = n_cols) of each issuing warp of block 0; synchronises."""
     out = torch.zeros(2, dtype=torch.int64, device="cuda")
@@ -242,10 +265,22 @@ def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, stream=None):
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
                  "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "mma_products", "mma_wait_failures",
-                 "seed_addbacks", "seeds")
+                 "seed_addbacks", "seeds", "mma_colsteps", "cluster_divs")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:
-    out = (ctypes.c_ulonglong * 16)()
+    out = (ctypes.c_ulonglong * NUM_COUNTERS)()
     _raise(lib().mpdiv_debug_counters(out, 1 if reset else 0, _stream_ptr(stream)), "mpdiv_debug_counters")
     return {k: int(out[i]) for i, k in enumerate(COUNTER_NAMES)}
+
+
+def status(reset: bool = False, stream=None) -> int:
+    """Sticky status bits of the current device (STATUS_*); synchronises the stream.  0 = all results exact."""
+    flags = ctypes.c_uint(0)
+    _raise(lib().mpdiv_status(_stream_ptr(stream), ctypes.byref(flags), 1 if reset else 0), "mpdiv_status")
+    return int(flags.value)
+
+
+def mma_probe_macs(n_cols: int, issuers: int, iters: int) -> int:
+    """u8 x u8 multiply-accumulates one mpdiv_mma_probe launch executes."""
+    return int(lib().mpdiv_mma_probe_macs(int(n_cols), int(issuers), int(iters)))

@@ -30,46 +30,11 @@
 
 namespace mpd {
 
-// debug counters (include/mpdiv.h: mpdiv_debug_counters)
-__device__ unsigned long long g_counters[16];
-enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
-       CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
-       CNT_MMA_PRODUCTS, CNT_MMA_WAIT_FAILURES /* filled by the host from mp_mma.cuh */, CNT_SEED_ADDBACK, CNT_SEEDS };
-
-// Phase timing for tuning builds only (-DMPDIV_PHASE_TIMING): thread 0 of block 0 accumulates the cycles
-// between consecutive PHASE() marks.  Compiles to nothing in the product build.
-#ifdef MPDIV_PHASE_TIMING
-__device__ unsigned long long g_op[16];
-#define OPDECL() long long tacc_[8] = {0,0,0,0,0,0,0,0}; long long tt_ = clock64()
-#define OPT(i) do { long long t__ = clock64(); tacc_[i] += t__ - tt_; tt_ = t__; } while (0)
-#define OPFLUSH() do { if (blockIdx.x == 0 && threadIdx.x == 0 && it >= 4 && it < 8) for (int i_ = 0; i_ < 8; i_++) atomicAdd(&g_op[i_], (unsigned long long)tacc_[i_]); } while (0)
-__device__ unsigned long long g_phase[64];
-__device__ long long g_phase_t0;
-#define PHASE(i)                                                        \
-    do {                                                                \
-        if (blockIdx.x == 0 && threadIdx.x == 0) {                      \
-            const long long t_ = clock64();                             \
-            g_phase[(i)] += (unsigned long long)(t_ - g_phase_t0);      \
-            g_phase_t0 = t_;                                            \
-        }                                                               \
-    } while (0)
-#else
-#define OPDECL() do { } while (0)
-#define OPT(i) do { } while (0)
-#define OPFLUSH() do { } while (0)
-#define PHASE(i) do { } while (0)
-#endif
-
 __device__ __forceinline__ void count_tiles(Blk &blk)
 {
     uint32_t t = __reduce_add_sync(0xffffffffu, blk.tiles);
     if ((threadIdx.x & 31) == 0 && t != 0) atomicAdd(&g_counters[CNT_TILES], (unsigned long long)t);
     blk.tiles = 0;
-}
-
-__device__ __forceinline__ void count(int which)
-{
-    if (threadIdx.x == 0) atomicAdd(&g_counters[which], 1ull);
 }
 
 // significant limbs of a shared-memory number known to have at most `bound` limbs.
@@ -131,9 +96,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     const int pv = k + 1 - s;
     const int hp = k + l + m - s + g;                      // h' of Step
     const int hpp = hp - m;                                // h'' of PowDiff
-    OPDECL(); 
     const int pw = top_prec(Wc, min(wlen, l + g + 2));
-    OPT(1);
     const int d = hp - 2 * m;                              // limbs of w*x that shift_{2m-h'} drops
 
     // ---- PowDiff (Alg. 2): (sign, x) = (B^h'' >= v'w, |B^h'' - v'w|) -------
@@ -144,7 +107,6 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     if (L >= hpp) {
         // no room to truncate: full product and a comparison with B^h''
         mul_full<TT>(Vp, pv, Wc, pw, P, ms, blk);
-        OPT(4);
         const int pl = round_up(pv, TILE) + round_up(pw, TILE);
         positive = !any_nonzero<TT>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
         if (positive) {
@@ -162,7 +124,6 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         if (Klo2 <= 0) {
             // close product: only the L low limbs of v'w (MULTMOD)
             mul_low<TT>(Vp, pv, Wc, pw, L, P, ms, blk);
-            OPT(4);
             positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
             xl = L;
             if (positive)
@@ -180,7 +141,6 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
                 c = TILE * Klo2;
                 mul_range<TT>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
             }
-            OPT(4);
             xl = L - c;
             positive = P[xl - 1] != 0u;
             for (int i = threadIdx.x; i < round_up(xl, TILE); i += TT)
@@ -189,10 +149,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         }
     }
     if (!positive) count(CNT_SIGN_NEG);
-    OPT(2);
     xl = top_prec(X, xl);
-    OPT(3);
-    PHASE(16 + (it & 15));
 
     // ---- Step (Alg. 1 lines 29-37): w <- shift_m(w) +- shift_{2m-h'}(w x), then shift_{-1} ----
     const int nlen = round_up(l + m + g + 2, TILE);
@@ -212,14 +169,12 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         if (tl >= 0) {
         } else if (Klo1 == 0) {
             mul_full<TT>(Wc, pw, X, xl, P, ms, blk);
-            OPT(5);
             tl = round_up(pw, TILE) + round_up(xl, TILE);
             off = dd;
         } else {
             tl = mul_range<TT>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
             off = dd - TILE * Klo1;
         }
-        OPT(5);
         if (positive) {
             lin_addsub<TT, false>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, 0u, blk);
         } else {
@@ -230,8 +185,6 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
             lin_addsub<TT, true>(Wn, nlen, LimbView{Wc, wlen, 1 - m}, LimbView{P, tl, off}, bin, blk);
         }
     }
-    OPT(7); OPFLUSH();
-    PHASE(32 + (it & 15));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -446,7 +399,6 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     __syncthreads();
 
     // ---- Refine (Alg. 1 lines 15-28) ------------------------------------------------------------
-    PHASE(0);
     // The early iterations (l <= NARROW_L: operands of at most ~40 x 70 limbs) run on warp 0 alone.
     // (narrow_l = 33 when the grid has more blocks than SMs: a lone block per SM is latency bound and keeps all
     // its threads; 0 disables)

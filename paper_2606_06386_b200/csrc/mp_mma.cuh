@@ -161,15 +161,9 @@ struct MmaCtx {
     uint32_t bar;         // shared address of the mbarriers: full[s] at +8 s, empty[s] at +64 + 8 s, done at +128
     uint32_t it;          // tiles produced so far (stage index and barrier parities follow from it)
     uint32_t ndone;       // products finished so far (parity of the done barrier)
-    uint32_t fail;        // set when a bounded wait gave up
+    uint32_t fail;        // set when a bounded wait gave up: the engine is retired for this block
 };
 
-#ifdef MMA_TIMING
-__device__ unsigned long long g_mma_t[8];
-#define MMA_T(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { long long t_ = clock64(); g_mma_t[i] += (unsigned long long)(t_ - t0_); t0_ = t_; } } while (0)
-#else
-#define MMA_T(i) do { } while (0)
-#endif
 __device__ unsigned int g_mma_fail;   // bounded waits that gave up (expected 0); reported with the debug counters
 
 constexpr int MMA_BAR_BYTES = 256;    // full[s] (up to 8), empty[s] (up to 8), done, TMEM slot
@@ -277,7 +271,7 @@ __device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
 template <int T>
 __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
 {
-    if (cx == nullptr || na <= 0 || nb <= 0 || dlo < 0) return false;
+    if (cx == nullptr || cx->fail || na <= 0 || nb <= 0 || dlo < 0) return false;
     dhi = min(dhi, (na + nb + 31) / 32);
     const int N = dhi - dlo, Nn = (N + 15) & ~15;
     if (N <= 0) return false;
@@ -301,7 +295,8 @@ __device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int d
 // A (na limbs) is the Toeplitz operand, B (nb limbs) the row operand; both plain little-endian limbs in
 // shared memory, read as zero beyond na / nb.  HI is scratch of the same size as P (+8).  dhi is clamped
 // to the size of the full product.  All T threads call it; ends with the result visible to the block.
-// Returns the number of limbs stored, or -1 when the request does not fit (TMEM columns or row buffer).
+// Returns the number of limbs stored, -1 when the request does not fit (TMEM columns or row buffer), -2 when a
+// bounded pipeline wait gave up (status bit set, engine retired; P holds nothing: redo the product elsewhere).
 template <int T>
 __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na, const limb *B, int nb, int dlo, int dhi,
                                           limb *P, limb *HI, Blk &blk)
@@ -318,9 +313,6 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     const int R = (dlo + Nn - 1 - pmin) - e0 + 1;
     if (N <= 0 || pmax < pmin || Nn > cx.acc_cols || R > cx.brows_cap) return -1;
 
-#ifdef MMA_TIMING
-    long long t0_ = clock64();
-#endif
     // ---- the row operand: chunk e of b -> row e - e0, 16-byte units swizzled by the row number ----
     for (int q = tid; q < R * 8; q += T) {
         const int r = q >> 3, c = q & 7;
@@ -334,8 +326,6 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     }
     fence_async_smem();
     __syncthreads();
-
-    MMA_T(0);
     const int nsteps = pmax - pmin + 1;
     using Roles = MmaRoles<T>;
     constexpr int G = Roles::GROUPS;
@@ -428,13 +418,11 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     }
     cx.it += (uint32_t)nsteps;
     __syncwarp();
-    MMA_T(1);
 
     // ---- epilogue: TMEM lane i, column d  ->  byte-column sum of output byte 128 (dlo + d) + i ----
     if (warp < 4) {
         if (!mbar_wait(cx.bar + 128, cx.ndone & 1)) cx.fail = 3;
         tc_fence_after();
-        MMA_T(2);
         for (int d0 = 0; d0 < Nn; d0 += 16) {
             uint32_t v[16];
             tmem_ld16(cx.tmem_base + ((uint32_t)(32 * warp) << 16) + d0, v);
@@ -453,16 +441,21 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
         if (tid == 0) HI[0] = 0u;
         tc_fence_before();
     }
-    MMA_T(3);
     cx.ndone += 1;
     if (cx.fail) atomicOr(&g_mma_fail, 1u << (cx.fail - 1));
-    __syncthreads();
+    if (__syncthreads_or(cx.fail != 0)) {
+        // a bounded wait gave up somewhere in the block: the accumulators cannot be trusted and the barrier
+        // parities are out of step.  Say so (sticky status bit), retire the engine for the rest of this block
+        // (mma_plan refuses a failed context) and let the caller redo this product on the IMAD path.
+        raise_status(ST_MMA_WAIT);
+        cx_mem.fail = 1;
+        return -2;
+    }
     // ---- P += HI with block-wide carry propagation (the carry out of the top block is dropped: mod B^(32 dhi)) ----
     lin_addsub<T, false>(P, 32 * N, LimbView{P, 32 * N, 0}, LimbView{HI, 32 * N, 0}, 0u, blk);
-    MMA_T(4);
     cx_mem.it = cx.it;
     cx_mem.ndone = cx.ndone;
-    cx_mem.fail = cx.fail;
+    count(CNT_MMA_COLSTEPS, (unsigned long long)nsteps * (unsigned long long)Nn);   // x 16384 = u8 MACs executed
     return 32 * N;
 }
 

@@ -25,22 +25,6 @@
 #pragma once
 #include "mp_block.cuh"
 
-// Tuning builds (-DMPDIV_PHASE_TIMING) split the cycles of block 0 by sub-phase; see mp_div.cuh.
-#ifdef MPDIV_PHASE_TIMING
-__device__ unsigned long long g_sub[64];
-__device__ long long g_sub_t0;
-#define SUBPHASE(i)                                                     \
-    do {                                                                \
-        if (blockIdx.x == 0 && threadIdx.x == 0) {                      \
-            const long long t_ = clock64();                             \
-            g_sub[(i)] += (unsigned long long)(t_ - g_sub_t0);          \
-            g_sub_t0 = t_;                                              \
-        }                                                               \
-    } while (0)
-#else
-#define SUBPHASE(i) do { } while (0)
-#endif
-
 namespace mpd {
 
 // four limb products of one parity class of row a: the 8-limb window held in the four 64-bit
@@ -353,11 +337,8 @@ __device__ __forceinline__ void mul_full(const limb *A, int na, const limb *Bp, 
 {
     const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
     const int Kd = Na + Nb - 1;
-    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, false);
-    SUBPHASE(49);
     blk.parity = mul_resolve<T>(P, 0, Kd, Na + Nb, ms.HI, ms.OV, ms.C3, blk);
-    SUBPHASE(50);
 }
 
 template <int T>
@@ -368,11 +349,8 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
     const int Kfull = Na + Nb;
     const int Kc = min((L + TILE - 1) / TILE, Kfull);
     const int Kd = min(Kc, Kfull - 1);
-    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, Kd < Kfull - 1);
-    SUBPHASE(49);
     blk.parity = mul_resolve<T>(P, 0, Kd, Kc, ms.HI, ms.OV, ms.C3, blk);
-    SUBPHASE(50);
 }
 
 // Clipped ("range") product: only tile diagonals Klo <= K < Khi are computed, so the result is
@@ -391,11 +369,8 @@ __device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, 
     const int Kd = min(Kc, Kfull - 1);
     limb *Pd = P - TILE * Klo, *HId = ms.HI - TILE * Klo;
     uint32_t *OVd = ms.OV - Klo, *C3d = ms.C3 - Klo;
-    SUBPHASE(48);
     blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, true);
-    SUBPHASE(49);
     blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
-    SUBPHASE(50);
     return TILE * max(Kc - Klo, 0);
 }
 

@@ -1,7 +1,10 @@
 // libmpdiv.so -- kernels and C ABI (include/mpdiv.h).  sm_100a only.
+#include <atomic>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
+#include <unordered_map>
 #include <cuda_runtime.h>
 
 #include "../../include/mpdiv.h"
@@ -11,7 +14,7 @@
 
 using namespace mpd;
 
-#define MPDIV_VERSION_STR "mpdiv 0.5 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
+#define MPDIV_VERSION_STR "mpdiv 0.6 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
 
 // ---------------------------------------------------------------------------------------
 // global <-> shared staging
@@ -216,47 +219,91 @@ imad_probe_kernel(uint32_t *sink, int iters)
 // ---------------------------------------------------------------------------------------
 namespace {
 
-int g_sm_count = 0;
-int g_max_smem = 0;
+// Per-device facts, cached on first use (any host thread, any device): the entry points call device_props()
+// first, which refreshes the thread-local copies for the CURRENT device.
+constexpr int MAX_DEVICES = 64;
+struct DevInfo { int sm_count, max_smem; };
+std::mutex g_host_mutex;                         // guards every lazily created library-owned host object
+DevInfo g_devinfo[MAX_DEVICES];
+std::atomic<bool> g_devinfo_ok[MAX_DEVICES];
+thread_local int g_dev = 0, g_sm_count = 0, g_max_smem = 0;
 
 bool device_props()
 {
-    if (g_sm_count > 0) return true;
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return false;
-    if (cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return false;
-    if (cudaDeviceGetAttribute(&g_max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
-        return false;
-    return g_sm_count > 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return false;
+    if (!g_devinfo_ok[dev].load(std::memory_order_acquire)) {
+        std::lock_guard<std::mutex> lk(g_host_mutex);
+        DevInfo d{0, 0};
+        if (cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return false;
+        if (cudaDeviceGetAttribute(&d.max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return false;
+        if (d.sm_count <= 0) return false;
+        g_devinfo[dev] = d;
+        g_devinfo_ok[dev].store(true, std::memory_order_release);
+    }
+    g_dev = dev;
+    g_sm_count = g_devinfo[dev].sm_count;
+    g_max_smem = g_devinfo[dev].max_smem;
+    return true;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// Tuning switches carried by the `flags` argument of the *_ex calls (include/mpdiv.h).
+struct Tune {
+    bool no_seed, no_head, no_mma, no_cluster;
+    int threads;                                 // 0 = by size
+};
+Tune tune_of(int flags)
+{
+    Tune t;
+    t.no_seed = (flags & MPDIV_FLAG_NO_SEED) != 0;
+    t.no_head = (flags & MPDIV_FLAG_NO_HEAD) != 0;
+    t.no_mma = (flags & MPDIV_FLAG_NO_MMA) != 0;
+    t.no_cluster = (flags & MPDIV_FLAG_NO_CLUSTER) != 0;
+    const int c = (flags & MPDIV_FLAG_THREADS_MASK) >> 8;
+    t.threads = c >= 1 && c <= 4 ? 32 << c : 0;
+    return t;
+}
+bool flags_ok(int flags)
+{
+    const int var = flags & MPDIV_VARIANT_MASK;
+    if (var != MPDIV_VARIANT_PRINTED && var != MPDIV_VARIANT_CLIPPED) return false;
+    if (flags & ~(MPDIV_VARIANT_MASK | MPDIV_FLAG_NO_SEED | MPDIV_FLAG_NO_HEAD | MPDIV_FLAG_NO_MMA | MPDIV_FLAG_NO_CLUSTER |
+                  MPDIV_FLAG_THREADS_MASK)) return false;
+    return ((flags & MPDIV_FLAG_THREADS_MASK) >> 8) <= 4;
+}
+
 // threads per block for numbers of `limbs` limbs.  Four lanes share a tile diagonal (mp_mul.cuh), so
 // a block of T threads covers T/4 diagonals = 2T limbs of product per pass.  256 threads at 128
 // registers let two blocks share an SM up to 4096 limbs; above that one block of 512 fills the SM.
-int threads_for(int limbs)
+int threads_for(int limbs, int override_threads = 0)
 {
-    if (const char *e = getenv("MPDIV_THREADS")) {     // tuning experiments only
-        const int t = atoi(e);
-        if (t == 64 || t == 128 || t == 256 || t == 512) return t;
-    }
+    if (override_threads) return override_threads;
     if (limbs <= 128) return 64;
     if (limbs <= 2048) return 128;      // four blocks per SM overlap the latency-bound early iterations
     if (limbs <= 4096) return 256;
     return 512;
 }
 
-template <class K>
-int set_smem(K kernel, size_t bytes)
+// Opt a kernel in to the device's full dynamic shared memory, once per kernel and device (the launch itself
+// states how much it uses, so occupancy is unaffected).
+int set_smem(const void *kernel, size_t bytes)
 {
     if ((int)bytes > g_max_smem) return MPDIV_ERR_UNSUPPORTED;
-    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) {
+    static std::unordered_map<const void *, unsigned long long> done;     // kernel -> mask of devices
+    std::lock_guard<std::mutex> lk(g_host_mutex);
+    unsigned long long &mask = done[kernel];
+    if (mask >> g_dev & 1ull) return MPDIV_OK;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem) != cudaSuccess) {
         cudaGetLastError();
         return MPDIV_ERR_CUDA;
     }
+    mask |= 1ull << g_dev;
     return MPDIV_OK;
 }
+template <class K>
+int set_smem(K kernel, size_t bytes) { return set_smem(reinterpret_cast<const void *>(kernel), bytes); }
 
 template <int T>
 int launch_mul(const limb *a, int a_limbs, const limb *b, int b_limbs, limb *c, int c_limbs, int batch,
@@ -369,14 +416,20 @@ mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
     mma_fini<128>(cx);
 }
 
+unsigned long long mpdiv_mma_probe_macs(int n_cols, int issuers, int iters)
+{
+    if (iters <= 0 || (issuers != 1 && issuers != 2) || n_cols < 16 || n_cols > 128 || (n_cols & 15) || !device_props())
+        return 0ull;
+    return (unsigned long long)g_sm_count * issuers * iters * 4ull * 128ull * (unsigned long long)n_cols * 32ull;
+}
+
 int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream)
 {
     if (!cycles || iters <= 0 || (issuers != 1 && issuers != 2) || n_cols < 16 || n_cols > 128 || (n_cols & 15))
         return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
     const int bytes = MMA_PROBE_ROWS * 128 + 1024;
-    if (cudaFuncSetAttribute(mma_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess)
-        return MPDIV_ERR_CUDA;
+    if (set_smem(mma_probe_kernel, (size_t)bytes) != MPDIV_OK) return MPDIV_ERR_CUDA;
     mma_probe_kernel<<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }

@@ -166,6 +166,7 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
         const int pv = prec_of<T>(V + 4, v_limbs, blk);
         if (pv == 0) {                                   // v = 0: undefined
             count(CNT_V_ZERO);
+            raise_status(ST_V_ZERO);
             for (int i = threadIdx.x; i < w_limbs; i += T) wout[i] = 0xffffffffu;
             __syncthreads();
             continue;
@@ -240,9 +241,6 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         limb *qg = q + (size_t)inst * u_limbs;
         limb *rg = r + (size_t)inst * v_limbs;
 
-#ifdef MPDIV_PHASE_TIMING
-        if (blockIdx.x == 0 && threadIdx.x == 0) g_phase_t0 = clock64();
-#endif
         // a1/a2: load, precisions ("h <- prec(u)")
         load_number<T>(V + 4, v + (size_t)inst * v_limbs, v_limbs, vpad - 4);
         load_number<T>(U + 4, ug, u_limbs, upad - 4);
@@ -253,6 +251,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         if (pv == 0) {                                     // v = 0: q = all ones, r = low limbs of u
             count(CNT_V_ZERO);
+            raise_status(ST_V_ZERO);
             for (int i = threadIdx.x; i < u_limbs; i += T) qg[i] = 0xffffffffu;
             store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
             __syncthreads();
@@ -279,11 +278,9 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
-        PHASE(1);
         const int nw = shinv_block<T, MMA>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256),
                                       (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
-        PHASE(2);
 
         // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
         if (one_limb) {
@@ -294,8 +291,6 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             load_number<T>(U + 4, ug, u_limbs, upad - 4);
         }
         __syncthreads();
-
-        PHASE(3);
         const int nq = h - k + 1;                          // q0 <= B^(h-k): at most h-k+1 limbs
         const int qlen = round_up(nq + 1, TILE);
         limb *Q = WA;
@@ -346,7 +341,6 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 }
             }
             const int pq = top_prec(Q, nq);
-            PHASE(4);
 
             // a10 clipped: |u - v q0'| < 4v < B^(k+2), so the remainder arithmetic runs mod B^rlen
             rlen = round_up(k + 3, TILE);
@@ -361,10 +355,10 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                     pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
                 }
             }
-
-            PHASE(5);
             // a11: r = u - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
             lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
+            // the estimate must lie in (-B^(k+2), B^(k+2)): its top limb (index >= k+2) is 0 or all ones
+            if (R[rlen - 1] != 0u && R[rlen - 1] != 0xffffffffu) raise_status(ST_REM_RANGE);
             while (R[rlen - 1] != 0u && minus < CORR_MAX) {
                 ++minus;
                 lin_addsub<T, false>(R, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
@@ -384,15 +378,16 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         }
         if (plus == 1) count(CNT_DELTA_POS);
         if (plus > 1) count(CNT_DELTA_MULTI);
-        if (plus >= CORR_MAX || minus >= CORR_MAX) count(CNT_DELTA_OUT_OF_RANGE);
-        PHASE(6);
+        if (plus >= CORR_MAX || minus >= CORR_MAX) {       // not exact: say so loudly (mpdiv_status)
+            count(CNT_DELTA_OUT_OF_RANGE);
+            raise_status(ST_CORR_BOUND);
+        }
 
         // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
         store_number<T>(qg, Q, u_limbs, min(qlen, u_limbs));
         if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
         else store_number<T>(rg, R, v_limbs, min(k + 1, v_limbs));
         __syncthreads();
-        PHASE(7);
     }
     count_tiles(blk);
     if constexpr (MMA) {
@@ -451,6 +446,8 @@ mplinop_kernel(int op, const limb *__restrict__ a, int a_limbs, const limb *__re
 // ---------------------------------------------------------------------------------------
 namespace {
 
+std::mutex g_host_call_mutex;          // serialises mpdiv_batch_host's enqueue (its calls share events)
+
 template <int T, bool E = MmaEnabled<T>::value>
 struct MmaStagesOf { static constexpr int value = 0; };
 template <int T>
@@ -459,22 +456,22 @@ struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; 
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 // low byte: l up to which Refine runs on warp 0 alone; bit 8: MPDIV_NO_SEED (tuning: start Refine at l = 2)
-int narrow_for(int batch) { return (batch > g_sm_count ? 33 : 0) | (getenv("MPDIV_NO_SEED") ? 256 : 0); }
+int narrow_for(int batch, const Tune &tn) { return (batch > g_sm_count ? 33 : 0) | (tn.no_seed ? 256 : 0); }
 
 // the head kernel pays off when the SMs hold several blocks each and Refine has iterations to hand over
 constexpr int HEAD_MIN_LIMBS = 512;
-static bool use_head(int u_limbs, int clip, bool lat)
+static bool use_head(int u_limbs, int clip, bool lat, const Tune &tn)
 {
-    return clip && !lat && u_limbs >= HEAD_MIN_LIMBS && !getenv("MPDIV_NO_HEAD") && !getenv("MPDIV_NO_SEED");
+    return clip && !lat && u_limbs >= HEAD_MIN_LIMBS && !tn.no_head && !tn.no_seed;
 }
 
 // Library-owned memory pool of the current device for the head's workspace rows: freed rows stay in the pool
 // (release threshold = everything), so a call costs a pool look-up, not a driver allocation.
 static cudaMemPool_t head_pool()
 {
-    static cudaMemPool_t pools[64] = {nullptr};
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    static cudaMemPool_t pools[MAX_DEVICES] = {nullptr};
+    const int dev = g_dev;                                   // set by device_props() of the calling entry point
+    std::lock_guard<std::mutex> lk(g_host_mutex);
     if (!pools[dev]) {
         cudaMemPoolProps props = {};
         props.allocType = cudaMemAllocationTypePinned;
@@ -492,7 +489,7 @@ static cudaMemPool_t head_pool()
 
 template <int T, bool LAT, bool MMA>
 int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-                 cudaStream_t st, int clip, int sched, bool tensor)
+                 cudaStream_t st, int clip, int sched, bool tensor, const Tune &tn)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     if (MMA && tensor) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
@@ -502,7 +499,7 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
     // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
     // iterate over in a stream-ordered workspace (mp_div.cuh "Head of Refine")
     limb *wmid = nullptr;
-    if (use_head(u_limbs, clip, LAT)) {
+    if (use_head(u_limbs, clip, LAT, tn)) {
         if (!head_pool() ||
             cudaMallocFromPoolAsync(reinterpret_cast<void **>(&wmid), (size_t)batch * WMID_STRIDE * sizeof(limb), head_pool(), st) != cudaSuccess) {
             cudaGetLastError();
@@ -511,7 +508,7 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
             shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
         }
     }
-    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched), wmid);
+    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched, tn), wmid);
     const bool ok = cudaGetLastError() == cudaSuccess;
     if (wmid) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
@@ -519,39 +516,40 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
 
 template <int T, bool LAT>
 int launch_div_k(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-                 cudaStream_t st, int clip, int sched)
+                 cudaStream_t st, int clip, int sched, const Tune &tn)
 {
     // tensor-core range products: clipped variant only; 128-thread blocks from 2^16 bits up (throughput batches of
     // 2^15 bits are faster on the IMAD path alone, 7.05 M against 6.64 M div/s, and run the instantiation without
     // the engine)
-    const bool tensor = DivMma<T, LAT>::value && clip && !(T <= 128 && u_limbs < 1536) && !getenv("MPDIV_NO_MMA");
+    const bool tensor = DivMma<T, LAT>::value && clip && !(T <= 128 && u_limbs < 1536) && !tn.no_mma;
     if constexpr (T == 128 && !LAT) {
-        if (!tensor) return launch_div_m<T, LAT, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, false);
+        if (!tensor) return launch_div_m<T, LAT, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, false, tn);
     }
-    return launch_div_m<T, LAT, DivMma<T, LAT>::value>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tensor);
+    return launch_div_m<T, LAT, DivMma<T, LAT>::value>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tensor, tn);
 }
 
 // sched = the number of divisions that share the GPU with this launch (the batch itself, or the whole batch
 // when the host path launches it chunk by chunk on several streams): it picks the kernel flavour.
 template <int T>
 int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
-               cudaStream_t st, int clip, int sched)
+               cudaStream_t st, int clip, int sched, const Tune &tn)
 {
     // a batch that fits the SMs at the latency kernel's occupancy (two blocks per SM up to 128 threads, one at
     // 256) is latency bound: give its threads all the registers they want
     if (T <= 256 && sched <= (T <= 128 ? 2 : 1) * g_sm_count)
-        return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
-    return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+        return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+    return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
 }
 
 template <int T>
-int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st, int clip)
+int launch_shinv(const limb *v, int v_limbs, int h, limb *w, int w_limbs, int batch, cudaStream_t st, int clip,
+                 const Tune &tn)
 {
     const DivLayout L = div_layout(h + 1, v_limbs, false, clip != 0);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(shinv_kernel<T>, bytes);
     if (rc != MPDIV_OK) return rc;
-    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L, clip, narrow_for(batch));
+    shinv_kernel<T><<<batch, T, bytes, st>>>(v, v_limbs, h, w, w_limbs, batch, L, clip, narrow_for(batch, tn));
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
@@ -560,8 +558,7 @@ int check_div_args(const void *u, int u_limbs, const void *v, int v_limbs, const
 {
     if (!u || !v || !q || !r || u_limbs <= 0 || v_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
     if ((u_limbs | v_limbs) & 3) return MPDIV_ERR_BAD_ARG;
-    if (v_limbs > u_limbs) return MPDIV_ERR_BAD_ARG;
-    if (u_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (u_limbs > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     return MPDIV_OK;
 }
 
@@ -576,39 +573,41 @@ int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, 
 }
 
 static int div_dispatch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
-                        int batch, int clip, cudaStream_t st, int sched)
+                        int batch, int clip, cudaStream_t st, int sched, const Tune &tn)
 {
-    switch (threads_for(u_limbs)) {
-        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
-        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
-        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
-        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched);
+    switch (threads_for(u_limbs, tn.threads)) {
+        case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+        case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+        case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+        default: return launch_div<512>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
     }
 }
 
 int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
-                   int batch, int variant, mpdiv_stream_t stream)
+                   int batch, int flags, mpdiv_stream_t stream)
 {
-    if (variant != MPDIV_VARIANT_PRINTED && variant != MPDIV_VARIANT_CLIPPED) return MPDIV_ERR_BAD_ARG;
-    const int clip = variant == MPDIV_VARIANT_CLIPPED;
+    if (!flags_ok(flags)) return MPDIV_ERR_BAD_ARG;
+    const int clip = (flags & MPDIV_VARIANT_MASK) == MPDIV_VARIANT_CLIPPED;
     int rc = check_div_args(u, u_limbs, v, v_limbs, q, r, batch);
     if (rc != MPDIV_OK) return rc;
     if (!aligned16(u) || !aligned16(v) || !aligned16(q) || !aligned16(r)) return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
-    return div_dispatch(u, u_limbs, v, v_limbs, q, r, batch, clip, reinterpret_cast<cudaStream_t>(stream), batch);
+    return div_dispatch(u, u_limbs, v, v_limbs, q, r, batch, clip, reinterpret_cast<cudaStream_t>(stream), batch, tune_of(flags));
 }
 
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch,
                 mpdiv_stream_t stream)
 {
-    return shinv_batch_ex(v, v_limbs, h, w, w_limbs, batch, MPDIV_VARIANT_DEFAULT, stream);
+    // Theorem 2's value, lambda in {0, 1}: the algorithm as printed
+    return shinv_batch_ex(v, v_limbs, h, w, w_limbs, batch, MPDIV_VARIANT_PRINTED, stream);
 }
 
-int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch, int variant,
+int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs, int batch, int flags,
                    mpdiv_stream_t stream)
 {
-    if (variant != MPDIV_VARIANT_PRINTED && variant != MPDIV_VARIANT_CLIPPED) return MPDIV_ERR_BAD_ARG;
-    const int clip = variant == MPDIV_VARIANT_CLIPPED;
+    if (!flags_ok(flags)) return MPDIV_ERR_BAD_ARG;
+    const int clip = (flags & MPDIV_VARIANT_MASK) == MPDIV_VARIANT_CLIPPED;
+    const Tune tn = tune_of(flags);
     if (!v || !w || v_limbs <= 0 || w_limbs <= 0 || batch <= 0 || h < 1) return MPDIV_ERR_BAD_ARG;
     if ((v_limbs | w_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (w_limbs < h + 1) return MPDIV_ERR_BAD_ARG;
@@ -616,11 +615,11 @@ int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_lim
     if (h > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    switch (threads_for(h)) {
-        case 64: return launch_shinv<64>(v, v_limbs, h, w, w_limbs, batch, st, clip);
-        case 128: return launch_shinv<128>(v, v_limbs, h, w, w_limbs, batch, st, clip);
-        case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st, clip);
-        default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st, clip);
+    switch (threads_for(h, tn.threads)) {
+        case 64: return launch_shinv<64>(v, v_limbs, h, w, w_limbs, batch, st, clip, tn);
+        case 128: return launch_shinv<128>(v, v_limbs, h, w, w_limbs, batch, st, clip, tn);
+        case 256: return launch_shinv<256>(v, v_limbs, h, w, w_limbs, batch, st, clip, tn);
+        default: return launch_shinv<512>(v, v_limbs, h, w, w_limbs, batch, st, clip, tn);
     }
 }
 
@@ -685,80 +684,85 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     const int chunk = (batch + nchunks - 1) / nchunks;
     nchunks = (batch + chunk - 1) / chunk;
 
-    static cudaStream_t s_in = nullptr, s_out = nullptr, s_k[NK];
-    static cudaEvent_t ev_start = nullptr, ev_in[MAXC], ev_k[MAXC], ev_done = nullptr;
-    if (!s_in) {
-        if (cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
-        if (cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
-        for (int i = 0; i < NK; i++)
-            if (cudaStreamCreateWithFlags(&s_k[i], cudaStreamNonBlocking) != cudaSuccess) return MPDIV_ERR_CUDA;
-        if (cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
-        if (cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
-        for (int i = 0; i < MAXC; i++) {
-            if (cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
-            if (cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming) != cudaSuccess) return MPDIV_ERR_CUDA;
+    // helper streams and events of the current device: created once, all or nothing, under the host lock;
+    // the lock also serialises the enqueue of concurrent calls (they share the events)
+    struct HostRes {
+        bool ok = false;
+        cudaStream_t s_in = nullptr, s_out = nullptr, s_k[NK] = {};
+        cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_in[MAXC] = {}, ev_k[MAXC] = {};
+    };
+    static HostRes res[MAX_DEVICES];
+    std::lock_guard<std::mutex> lk(g_host_call_mutex);
+    HostRes &hr = res[g_dev];
+    if (!hr.ok) {
+        HostRes t;
+        bool good = cudaStreamCreateWithFlags(&t.s_in, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaStreamCreateWithFlags(&t.s_out, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&t.ev_start, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&t.ev_done, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; good && i < NK; i++) good = cudaStreamCreateWithFlags(&t.s_k[i], cudaStreamNonBlocking) == cudaSuccess;
+        for (int i = 0; good && i < MAXC; i++)
+            good = cudaEventCreateWithFlags(&t.ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+                   cudaEventCreateWithFlags(&t.ev_k[i], cudaEventDisableTiming) == cudaSuccess;
+        if (!good) {                                          // nothing half-made survives
+            cudaGetLastError();
+            if (t.s_in) cudaStreamDestroy(t.s_in);
+            if (t.s_out) cudaStreamDestroy(t.s_out);
+            if (t.ev_start) cudaEventDestroy(t.ev_start);
+            if (t.ev_done) cudaEventDestroy(t.ev_done);
+            for (int i = 0; i < NK; i++) if (t.s_k[i]) cudaStreamDestroy(t.s_k[i]);
+            for (int i = 0; i < MAXC; i++) {
+                if (t.ev_in[i]) cudaEventDestroy(t.ev_in[i]);
+                if (t.ev_k[i]) cudaEventDestroy(t.ev_k[i]);
+            }
+            return MPDIV_ERR_CUDA;
         }
+        t.ok = true;
+        hr = t;
     }
-#define MPDIV_CK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return MPDIV_ERR_CUDA; } } while (0)
-    MPDIV_CK(cudaEventRecord(ev_start, st));                  // the helpers start after earlier work on `stream`
-    MPDIV_CK(cudaStreamWaitEvent(s_in, ev_start, 0));
+    // on an error part of the batch may be in flight on the helper streams: wait for it, so that the caller may
+    // reuse or free its buffers as soon as the call has returned
+    auto fail = [&](int code) {
+        cudaGetLastError();
+        cudaStreamSynchronize(hr.s_in);
+        for (int i = 0; i < NK; i++) cudaStreamSynchronize(hr.s_k[i]);
+        cudaStreamSynchronize(hr.s_out);
+        cudaGetLastError();
+        return code;
+    };
+#define MPDIV_CK(x) do { if ((x) != cudaSuccess) return fail(MPDIV_ERR_CUDA); } while (0)
+    const Tune tn = tune_of(0);
+    MPDIV_CK(cudaEventRecord(hr.ev_start, st));               // the helpers start after earlier work on `stream`
+    MPDIV_CK(cudaStreamWaitEvent(hr.s_in, hr.ev_start, 0));
     for (int c = 0; c < nchunks; c++) {
         const size_t lo = (size_t)c * chunk;
         const int cnt = (int)((size_t)batch - lo < (size_t)chunk ? (size_t)batch - lo : (size_t)chunk);
         const size_t uo = lo * u_limbs, vo = lo * v_limbs;
-        cudaStream_t sk = s_k[c % NK];
-        MPDIV_CK(cudaMemcpyAsync(du + uo, u_host + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyHostToDevice, s_in));
-        MPDIV_CK(cudaMemcpyAsync(dv + vo, v_host + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyHostToDevice, s_in));
-        MPDIV_CK(cudaEventRecord(ev_in[c], s_in));
-        MPDIV_CK(cudaStreamWaitEvent(sk, ev_in[c], 0));       // ev_in follows ev_start on s_in
-        rc = div_dispatch(du + uo, u_limbs, dv + vo, v_limbs, dq + uo, dr + vo, cnt, 1, sk, batch);
-        if (rc != MPDIV_OK) return rc;
-        MPDIV_CK(cudaEventRecord(ev_k[c], sk));
-        MPDIV_CK(cudaStreamWaitEvent(s_out, ev_k[c], 0));
-        MPDIV_CK(cudaMemcpyAsync(q_host + uo, dq + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyDeviceToHost, s_out));
-        MPDIV_CK(cudaMemcpyAsync(r_host + vo, dr + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyDeviceToHost, s_out));
+        cudaStream_t sk = hr.s_k[c % NK];
+        MPDIV_CK(cudaMemcpyAsync(du + uo, u_host + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyHostToDevice, hr.s_in));
+        MPDIV_CK(cudaMemcpyAsync(dv + vo, v_host + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyHostToDevice, hr.s_in));
+        MPDIV_CK(cudaEventRecord(hr.ev_in[c], hr.s_in));
+        MPDIV_CK(cudaStreamWaitEvent(sk, hr.ev_in[c], 0));    // ev_in follows ev_start on s_in
+        rc = div_dispatch(du + uo, u_limbs, dv + vo, v_limbs, dq + uo, dr + vo, cnt, 1, sk, batch, tn);
+        if (rc != MPDIV_OK) return fail(rc);
+        MPDIV_CK(cudaEventRecord(hr.ev_k[c], sk));
+        MPDIV_CK(cudaStreamWaitEvent(hr.s_out, hr.ev_k[c], 0));
+        MPDIV_CK(cudaMemcpyAsync(q_host + uo, dq + uo, (size_t)cnt * u_limbs * 4, cudaMemcpyDeviceToHost, hr.s_out));
+        MPDIV_CK(cudaMemcpyAsync(r_host + vo, dr + vo, (size_t)cnt * v_limbs * 4, cudaMemcpyDeviceToHost, hr.s_out));
     }
-    MPDIV_CK(cudaEventRecord(ev_done, s_out));                // s_out has waited for every chunk kernel
-    MPDIV_CK(cudaStreamWaitEvent(st, ev_done, 0));            // `stream` completes when the last download has
+    MPDIV_CK(cudaEventRecord(hr.ev_done, hr.s_out));          // s_out has waited for every chunk kernel
+    MPDIV_CK(cudaStreamWaitEvent(st, hr.ev_done, 0));         // `stream` completes when the last download has
 #undef MPDIV_CK
     return MPDIV_OK;
 }
 
-#ifdef MPDIV_PHASE_TIMING
-int mpdiv_debug_phases(unsigned long long out[64], int reset)
+int mpdiv_batch_launches(int u_limbs, int batch, int flags)
 {
-    if (cudaDeviceSynchronize() != cudaSuccess) return MPDIV_ERR_CUDA;
-    unsigned long long sub[64];
-    if (cudaMemcpyFromSymbol(out, g_phase, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
-    if (cudaMemcpyFromSymbol(sub, g_sub, 64 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
-    for (int i = 48; i < 64; i++) out[i] = sub[i];       // slots 48.. carry the multiplier sub-phases
-    unsigned long long op[16];
-    if (cudaMemcpyFromSymbol(op, g_op, sizeof(op)) != cudaSuccess) return MPDIV_ERR_CUDA;
-    for (int i = 0; i < 8; i++) out[8 + i] = op[i];      // slots 8..15: op-level split of Refine iterations 0..5
-    if (reset) { unsigned long long zz[16] = {0}; cudaMemcpyToSymbol(g_op, zz, sizeof(zz)); }
-#ifdef MMA_TIMING
-    {   // slots 56..63: tensor-core multiplier sub-phases (row operand, MMA loop, wait, epilogue, final add)
-        unsigned long long mt[8];
-        if (cudaMemcpyFromSymbol(mt, g_mma_t, sizeof(mt)) != cudaSuccess) return MPDIV_ERR_CUDA;
-        for (int i = 0; i < 8; i++) out[56 + i] = mt[i];
-        if (reset) { unsigned long long zz[8] = {0}; cudaMemcpyToSymbol(g_mma_t, zz, sizeof(zz)); }
-    }
-#endif
-    if (reset) {
-        unsigned long long z[64] = {0};
-        if (cudaMemcpyToSymbol(g_phase, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
-        if (cudaMemcpyToSymbol(g_sub, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
-    }
-    return MPDIV_OK;
-}
-#endif
-
-int mpdiv_batch_launches(int u_limbs, int batch, int variant)
-{
-    if (u_limbs <= 0 || batch <= 0 || !device_props()) return 0;
-    const int T = threads_for(u_limbs);
+    if (u_limbs <= 0 || batch <= 0 || !flags_ok(flags) || !device_props()) return 0;
+    const Tune tn = tune_of(flags);
+    const int T = threads_for(u_limbs, tn.threads);
     const bool lat = T <= 256 && batch <= (T <= 128 ? 2 : 1) * g_sm_count;
-    return use_head(u_limbs, variant == MPDIV_VARIANT_CLIPPED, lat) ? 2 : 1;
+    return use_head(u_limbs, (flags & MPDIV_VARIANT_MASK) == MPDIV_VARIANT_CLIPPED, lat, tn) ? 2 : 1;
 }
 
 int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpdiv_stream_t stream)
@@ -769,20 +773,35 @@ int mpdiv_seed_batch(const uint32_t *v, int v_limbs, uint32_t *w, int batch, mpd
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
-int mpdiv_debug_counters(unsigned long long out[16], int reset, mpdiv_stream_t stream)
+int mpdiv_debug_counters(unsigned long long out[MPDIV_NUM_COUNTERS], int reset, mpdiv_stream_t stream)
 {
+    static_assert(MPDIV_NUM_COUNTERS == NUM_COUNTERS, "header and device counters agree");
     if (!out) return MPDIV_ERR_BAD_ARG;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     if (cudaStreamSynchronize(st) != cudaSuccess) return MPDIV_ERR_CUDA;
-    if (cudaMemcpyFromSymbol(out, g_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(out, g_counters, NUM_COUNTERS * sizeof(unsigned long long)) != cudaSuccess) return MPDIV_ERR_CUDA;
     unsigned int mma_fail = 0;
     if (cudaMemcpyFromSymbol(&mma_fail, g_mma_fail, sizeof(mma_fail)) != cudaSuccess) return MPDIV_ERR_CUDA;
-    out[13] = mma_fail;
+    out[CNT_MMA_WAIT_FAILURES] = mma_fail;
     if (reset) {
         const unsigned int zf = 0;
         if (cudaMemcpyToSymbol(g_mma_fail, &zf, sizeof(zf)) != cudaSuccess) return MPDIV_ERR_CUDA;
-        unsigned long long z[16] = {0};
+        unsigned long long z[NUM_COUNTERS] = {0};
         if (cudaMemcpyToSymbol(g_counters, z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    }
+    return MPDIV_OK;
+}
+
+int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset)
+{
+    static_assert(MPDIV_STATUS_MMA_WAIT == ST_MMA_WAIT && MPDIV_STATUS_CORR_BOUND == ST_CORR_BOUND &&
+                  MPDIV_STATUS_REM_RANGE == ST_REM_RANGE && MPDIV_STATUS_V_ZERO == ST_V_ZERO, "status bits agree");
+    if (!flags) return MPDIV_ERR_BAD_ARG;
+    if (cudaStreamSynchronize(reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(flags, g_status, sizeof(unsigned int)) != cudaSuccess) return MPDIV_ERR_CUDA;
+    if (reset) {
+        const unsigned int z = 0;
+        if (cudaMemcpyToSymbol(g_status, &z, sizeof(z)) != cudaSuccess) return MPDIV_ERR_CUDA;
     }
     return MPDIV_OK;
 }

@@ -35,3 +35,26 @@ def max_over_ranks(value: float, device=None) -> float:
 def aggregate_rate(units_per_rank: int, world: int, ms_max: float) -> float:
     """Whole-job throughput: units all ranks processed divided by the slowest rank's time."""
     return world * units_per_rank / (ms_max * 1e-3)
+
+
+def free_port() -> int:
+    import socket
+
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def torchrun_argv(nproc: int, script: str, script_args, port: int | None = None, python: str | None = None) -> list:
+    """Command line that starts `script` as `nproc` ranks of one node, one process per GPU, rendezvous on
+    127.0.0.1 (the container hostname may not resolve): what `bench.py --gpus N` runs when it was not itself
+    started under torchrun."""
+    import sys
+
+    if nproc < 1:
+        raise ValueError("nproc must be >= 1")
+    return [python or sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(int(nproc)),
+            "--master-addr", "127.0.0.1", "--master-port", str(port if port is not None else free_port()),
+            script] + list(script_args)

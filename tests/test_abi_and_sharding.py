@@ -44,7 +44,9 @@ def test_bad_arguments_rejected_before_any_cuda_call():
     assert lib.mpdiv_batch(p, 6, p, 4, p, p, 1, null) == binding.ERR_BAD_ARG          # stride % 4
     assert lib.mpdiv_batch(p, 8, p, 4, p, p, 0, null) == binding.ERR_BAD_ARG          # empty batch
     assert lib.mpdiv_batch(p + 4, 8, p, 4, p, p, 1, null) == binding.ERR_BAD_ARG      # misaligned
-    assert lib.mpdiv_batch(p, 4, p, 8, p, p, 1, null) == binding.ERR_BAD_ARG          # v_limbs > u_limbs
+    assert lib.mpdiv_batch_ex(p, 8, p, 4, p, p, 1, 7, null) == binding.ERR_BAD_ARG    # unknown variant
+    assert lib.mpdiv_batch_ex(p, 8, p, 4, p, p, 1, 0x1000, null) == binding.ERR_BAD_ARG   # unknown flag bit
+    assert lib.mpdiv_batch(p, 8, p, 8196, p, p, 1, null) == binding.ERR_UNSUPPORTED    # v stride above the maximum
     assert lib.mpdiv_batch(p, 8196, p, 4, p, p, 1, null) == binding.ERR_UNSUPPORTED
     assert lib.mpmul_batch(p, 8, p, 8, p, 20, 1, null) == binding.ERR_BAD_ARG         # c_limbs > a+b
     assert lib.shinv_batch(p, 8, 16, p, 16, 1, null) == binding.ERR_BAD_ARG           # w_limbs < h+1
@@ -105,3 +107,42 @@ def test_two_rank_gloo_sharding_and_max_time():
     assert ms == 15.0                       # the slower rank's time
     assert abs(rate - 2 * 1184 / 15e-3) < 1e-6
     assert seed == 8
+
+
+def test_bench_spawns_its_own_ranks_with_torchrun():
+    """`python bench.py --gpus N` without WORLD_SIZE re-executes itself under torchrun (shard.torchrun_argv); the
+    same command line is run here on a CPU probe with the gloo backend and world size 2."""
+    import json
+    import subprocess
+    import sys
+
+    argv = shard.torchrun_argv(2, os.path.join(ROOT, "tests", "dist_probe.py"), ["--gpus", "2", "--steps", "3"])
+    assert argv[:3] == [sys.executable, "-m", "torch.distributed.run"] and "127.0.0.1" in argv
+    assert argv[argv.index("--nproc-per-node") + 1] == "2"
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    proc = subprocess.run(argv, capture_output=True, text=True, timeout=240, env=env)
+    assert proc.returncode == 0, proc.stderr[-2000:]
+    line = [ln for ln in proc.stdout.splitlines() if ln.startswith("{")][-1]
+    out = json.loads(line)
+    assert out["n_gpus"] == 2 and out["ms"] == 11.0 and out["first"] == [0, 592]
+    assert out["args"] == ["--gpus", "2", "--steps", "3"] and out["master"] == "127.0.0.1"
+    with pytest.raises(ValueError):
+        shard.torchrun_argv(0, "x.py", [])
+
+
+def test_bench_main_takes_the_spawn_path_only_without_world_size(monkeypatch):
+    """bench.main() spawns ranks iff --gpus > 1 and it is not already a rank (WORLD_SIZE unset)."""
+    import importlib
+    import subprocess
+    import sys
+
+    sys.path.insert(0, ROOT)
+    bench = importlib.import_module("bench")
+    calls = []
+    monkeypatch.setattr(subprocess, "call", lambda argv: calls.append(argv) or 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4", "--steps", "2", "--warmup", "1"])
+    with pytest.raises(SystemExit) as e:
+        bench.main()
+    assert e.value.code == 0 and len(calls) == 1
+    assert calls[0][calls[0].index("--nproc-per-node") + 1] == "4" and calls[0][-6:] == ["--gpus", "4", "--steps", "2", "--warmup", "1"]

@@ -2,8 +2,9 @@
 
 Every test here needs a B200 (``-m gpu``).  Inputs come from the seeded generators of
 ``paper_2606_06386_b200.inputs``; expected values come from ``oracle/`` only.  q and r are
-unique, so every limb including the zero padding must match.  For shinv the
-two admissible values floor(B^h/v) + {0, 1} (Theorem 2) are both accepted.
+unique, so every limb including the zero padding must match.  For shinv_batch the
+two admissible values floor(B^h/v) + {0, 1} (Theorem 2) are both accepted; the clipped
+variant behind shinv_batch_ex may also return floor(B^h/v) - 1.
 """
 import os
 
@@ -31,9 +32,14 @@ PRINTED, CLIPPED = binding.VARIANT_PRINTED, binding.VARIANT_CLIPPED
 VARIANTS = [pytest.param(CLIPPED, id="clipped"), pytest.param(PRINTED, id="printed")]
 
 
-def gpu_div(u, v, variant=None):
+def gpu_div(u, v, variant=None, allow=0):
+    """One batch through the C ABI; afterwards the sticky status word must be clean (mpdiv_status: no pipeline
+    wait gave up, no correction loop hit its bound, the clipped remainder stayed in range), except for the
+    bits in `allow` (a test that feeds v = 0 allows STATUS_V_ZERO)."""
+    binding.status(reset=True)
     q, r = binding.mpdiv_batch(dev(u), dev(v), variant=variant)
-    torch.cuda.synchronize()
+    st = binding.status(reset=True)
+    assert st & ~allow == 0, "mpdiv_status = %#x after the batch" % st
     return host(q), host(r)
 
 
@@ -121,19 +127,25 @@ def test_div_uses_tensor_engine_at_2_18_bits():
 # ------------------------------------------------------------------ shifted inverse
 @pytest.mark.parametrize("vn,h", [(4, 7), (8, 16), (16, 17), (64, 128), (512, 1024), (1024, 2048),
                                   (260, 777), (2048, 4096), (4096, 8192), (512, 512), (512, 300)])
-@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("variant", [pytest.param(None, id="plain"), pytest.param(CLIPPED, id="clipped-ex"),
+                                     pytest.param(PRINTED, id="printed-ex")])
 def test_shinv_parity(vn, h, variant):
+    """shinv_batch (no flags) is Theorem 2's value: lambda in {0, 1} ONLY."""
     batch = 24
     wn = (h + 1 + 3) // 4 * 4
     _, v = inputs.directed(max(vn, 8), vn, count=batch, seed=inputs.SEED + h)
     v2 = inputs._uniform(inputs.rng_for(201, h % 65536), 8, vn)
     inputs._force_top_nonzero(v2)
     v = np.concatenate([v, v2])
+    binding.status(reset=True)
     w = host(binding.shinv_batch(dev(v), h, wn, variant=variant))
+    assert binding.status(reset=True) & ~binding.STATUS_V_ZERO == 0
     wo = oracle.shinv_batch(v, h, wn)
-    allowed = (0, 1) if variant == PRINTED else (-1, 0, 1)      # Theorem 2; one more unit when clipped
+    allowed = (-1, 0, 1) if variant == CLIPPED else (0, 1)      # Theorem 2; one more unit when clipped
     lam_hist = {-1: 0, 0: 0, 1: 0}
     for i in range(v.shape[0]):
+        if not v[i].any():
+            continue                                            # v = 0: undefined (all ones, status bit)
         lam = inputs.from_limbs(w[i]) - inputs.from_limbs(wo[i])
         assert lam in allowed, "instance %d: lambda = %d (allowed %s)" % (i, lam, allowed)
         lam_hist[lam] += 1
@@ -308,12 +320,38 @@ def test_div_zero_divisor_does_not_trap():
     binding.debug_counters(reset=True)
     u, v = inputs.uniform_operands(8, 64, 32, config=77)
     v[3] = 0
-    q, r = gpu_div(u, v)
+    binding.status(reset=True)
+    binding.mpdiv_batch(dev(u), dev(v))
+    assert binding.status(reset=True) == binding.STATUS_V_ZERO      # undefined input is reported, not hidden
+    q, r = gpu_div(u, v, allow=binding.STATUS_V_ZERO)
     assert (q[3] == 0xFFFFFFFF).all() and (r[3] == u[3, :32]).all()
     keep = [0, 1, 2, 4, 5, 6, 7]
     qo, ro = oracle.divmod_batch(u[keep], v[keep])
     assert (q[keep] == qo).all() and (r[keep] == ro).all()
     assert binding.debug_counters(reset=True)["v_zero"] == 1
+
+
+@pytest.mark.parametrize("M,n", [(8, 16), (64, 128), (512, 1024), (2048, 4096), (1024, 8192)])
+def test_div_divisor_stride_longer_than_dividend(M, n):
+    """v_limbs > u_limbs is allowed: a divisor that is really longer gives (0, u); one whose
+    effective precision fits inside u's stride divides as usual.  r has the divisor's stride."""
+    rng = inputs.rng_for(420, n % 65536)
+    us, vs = [], []
+    for i in range(96):
+        lu = int(rng.integers(0, M + 1))
+        lv = int(rng.integers(1, n + 1)) if i % 2 else int(rng.integers(1, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, lv))
+    u, v = inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, n)
+    q, r = gpu_div(u, v)
+    assert q.shape == (96, M) and r.shape == (96, n)
+    for i in range(96):
+        qi, ri = divmod(us[i], vs[i])          # Python integers: the strides differ, so the limb oracle is
+        assert inputs.from_limbs(q[i]) == qi and inputs.from_limbs(r[i]) == ri, i   # called below on the padded u
+    up = np.zeros((96, n), dtype=np.uint32)
+    up[:, :M] = u
+    qo, ro = oracle.divmod_batch(up, v, threads=NCPU)
+    assert (qo[:, :M] == q).all() and not qo[:, M:].any() and (ro == r).all()
 
 
 def test_host_buffer_form_matches():

@@ -99,9 +99,9 @@ def test_seed_extremes():
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 5])
-def test_division_same_with_and_without_seed(cfg, monkeypatch):
-    """MPDIV_NO_SEED starts Refine at l = 2 as printed; q and r must not change (both are exact), and the shifted
-    inverse may differ by its lambda only."""
+def test_division_same_with_and_without_seed(cfg):
+    """MPDIV_FLAG_NO_SEED starts Refine at l = 2 as printed; q and r must not change (both are exact), and the
+    shifted inverse may differ by its lambda only."""
     import torch
 
     from paper_2606_06386_b200 import binding
@@ -113,9 +113,8 @@ def test_division_same_with_and_without_seed(cfg, monkeypatch):
     q1, r1 = binding.mpdiv_batch(du, dv)
     torch.cuda.synchronize()
     assert binding.debug_counters()["seeds"] > 0
-    monkeypatch.setenv("MPDIV_NO_SEED", "1")
     binding.debug_counters(reset=True)
-    q0, r0 = binding.mpdiv_batch(du, dv)
+    q0, r0 = binding.mpdiv_batch(du, dv, variant=binding.VARIANT_CLIPPED | binding.FLAG_NO_SEED)
     torch.cuda.synchronize()
     assert binding.debug_counters()["seeds"] == 0
     assert torch.equal(q0, q1) and torch.equal(r0, r1)
@@ -123,15 +122,16 @@ def test_division_same_with_and_without_seed(cfg, monkeypatch):
 
 # ---- the head of Refine in its own kernel (csrc/mp_div.cuh "Head of Refine") ------------------------------
 
-def _div(u, v):
+def _div(u, v, flags=None):
     import torch
 
     from paper_2606_06386_b200 import binding
 
     du = torch.from_numpy(u.view(np.int32)).cuda()
     dv = torch.from_numpy(v.view(np.int32)).cuda()
-    q, r = binding.mpdiv_batch(du, dv)
-    torch.cuda.synchronize()
+    binding.status(reset=True)
+    q, r = binding.mpdiv_batch(du, dv, variant=flags)
+    assert binding.status(reset=True) == 0
     return q.cpu().numpy().view(np.uint32), r.cpu().numpy().view(np.uint32)
 
 
@@ -147,7 +147,7 @@ def test_batch_launches_reports_the_head_kernel():
 
 
 @pytest.mark.parametrize("M,count", [(512, 1500), (1024, 900), (2048, 700), (4096, 400)])
-def test_head_kernel_random_precisions(M, count, monkeypatch):
+def test_head_kernel_random_precisions(M, count):
     """Batches large enough for the head kernel, random effective precisions of u and v: every H = h - k from
     below the seed's threshold (17) through every split point of head_plan occurs.  q and r against the oracle,
     and identical with the head switched off."""
@@ -172,8 +172,7 @@ def test_head_kernel_random_precisions(M, count, monkeypatch):
     assert cnt["seeds"] > 0 and cnt["delta_out_of_range"] == 0
     qo, ro = oracle.divmod_batch(u, v)
     assert (q1 == qo).all() and (r1 == ro).all()
-    monkeypatch.setenv("MPDIV_NO_HEAD", "1")
-    q0, r0 = _div(u, v)
+    q0, r0 = _div(u, v, binding.VARIANT_CLIPPED | binding.FLAG_NO_HEAD)
     assert (q0 == q1).all() and (r0 == r1).all()
 
 
