@@ -207,10 +207,12 @@ def measure_mma_issue(binding):
     """Cycles per tcgen05.mma (M = 128, K = 32, u8) seen by one issuing warp and by two (mpdiv_mma_probe): the
     tensor core needs N / 2; the rest is the issue path."""
     out = {}
-    for n in (16, 64, 128):
+    for n in (16, 48, 64, 96, 128):
         one = binding.mma_probe(n, 1)
         two = binding.mma_probe(n, 2)
+        ss = binding.mma_probe(n, 1, form=1)
         out["N=%d" % n] = {"one_warp_cycles_per_mma": one[0], "two_warps_cycles_per_mma_together": max(two) / 2.0,
+                           "toeplitz_descriptor_form_cycles_per_mma": ss[0], "shared_memory_model_cycles": max(32 + n / 4.0, n / 2.0),
                            "tensor_core_cycles_per_mma": n / 2.0}
     return out
 

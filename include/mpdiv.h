@@ -197,6 +197,9 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
  * Tensor-core issue-rate probe and int8 roofline probe: one 128-thread block per SM in which
  * `issuers` warps (1 or 2) each issue `iters` steps of four tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols,
  * 16 <= n_cols <= 128, multiple of 16) into their own accumulator columns, the way the multiplier issues them.
+ * form 0: the A operand in tensor memory (the pure rate of the pipe); form 1: A read from shared memory through
+ * the overlapped Toeplitz descriptor of csrc/mp_mma.cuh (what the multiplier issues: 32 cycles of shared-memory
+ * bandwidth per instruction, so max(32 + n_cols/4, n_cols/2) cycles).
  * cycles (DEVICE pointer, 2 words): SM cycles block 0's warp w needed for its 4 * iters instructions, 0 if a
  * bounded wait gave up.  The tensor core needs n_cols / 2 cycles per instruction; what a single warp measures
  * above that is its own issue path.  One launch executes  SMs x issuers x iters x 4 x 128 x n_cols x 32
@@ -204,7 +207,7 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
  * gives the measured peak of the tensor pipe for this data type.  Asynchronous on `stream`.
  */
 unsigned long long mpdiv_mma_probe_macs(int n_cols, int issuers, int iters);
-int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream);
+int mpdiv_mma_probe(int n_cols, int issuers, int iters, int form, unsigned long long *cycles, mpdiv_stream_t stream);
 
 /*
  * Status word of the current device: sticky bits set by the kernels since the last reset.  Synchronises

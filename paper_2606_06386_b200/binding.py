@@ -63,7 +63,7 @@ def lib() -> ctypes.CDLL:
         L.mpdiv_batch_host.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP, sz, _VOIDP]
         L.mpdiv_imad_probe_threads.argtypes = []
         L.mpdiv_imad_probe.argtypes = [_VOIDP, i, i, ctypes.POINTER(ctypes.c_ulonglong), _VOIDP]
-        L.mpdiv_mma_probe.argtypes = [i, i, i, _VOIDP, _VOIDP]
+        L.mpdiv_mma_probe.argtypes = [i, i, i, i, _VOIDP, _VOIDP]
         L.mpdiv_mma_probe.restype = i
         L.mpdiv_mma_probe_macs.argtypes = [i, i, i]
         L.mpdiv_mma_probe_macs.restype = ctypes.c_ulonglong
@@ -248,16 +248,17 @@ def imad_probe(kind: int, iters: int, sink: torch.Tensor | None = None, stream=N
     return int(prod.value), sink
 
 
-def mma_probe_launch(n_cols: int, issuers: int, iters: int, out: torch.Tensor, stream=None):
+def mma_probe_launch(n_cols: int, issuers: int, iters: int, out: torch.Tensor, form: int = 0, stream=None):
     """Enqueue one probe launch (no synchronisation): for timing with events."""
-    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), out.data_ptr(), _stream_ptr(stream)),
+    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), int(form), out.data_ptr(), _stream_ptr(stream)),
            "mpdiv_mma_probe")
 
 
-def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, stream=None):
-    """Cycles per tcgen05.mma (M = 128, K = 32, u8, N = n_cols) of each issuing warp of block 0; synchronises."""
+def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, form: int = 0, stream=None):
+    """Cycles per tcgen05.mma (M = 128, K = 32, u8, N = n_cols) of each issuing warp of block 0; synchronises.
+    form 0: A in tensor memory; form 1: A from shared memory through the Toeplitz descriptor."""
     out = torch.zeros(2, dtype=torch.int64, device="cuda")
-    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), out.data_ptr(), _stream_ptr(stream)),
+    _raise(lib().mpdiv_mma_probe(int(n_cols), int(issuers), int(iters), int(form), out.data_ptr(), _stream_ptr(stream)),
            "mpdiv_mma_probe")
     torch.cuda.synchronize()
     return [c / (4.0 * iters) for c in out.tolist()[:issuers]]

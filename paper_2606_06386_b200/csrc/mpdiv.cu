@@ -82,9 +82,9 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
     const int full = (a_limbs + b_limbs + 31) / 32, want = (c_limbs + 31) / 32;
     const int blocks = want < full ? want : full;
     const int nn = (blocks + 15) & ~15;
-    const int need = nn + 6 * MMA_STAGE_COLS;                           // accumulators + up to six Toeplitz stages
-    if (need > 512) return false;
-    const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
+    if (nn > 512) return false;
+    const int sets = 2 * nn;                                     // one accumulator set per issuing warp when they fit
+    const int cols = sets <= 32 ? 32 : sets <= 64 ? 64 : sets <= 128 ? 128 : sets <= 256 ? 256 : 512;
     const int small = a_limbs < b_limbs ? a_limbs : b_limbs;
     const int rows = round_up(nn + (small + 31) / 32 + 8, 8);
     // P and HI must hold 32 limbs per output block
@@ -100,7 +100,7 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
         L.total_words = o;
     }
     const int off = round_up(L.total_words, 256);
-    const int words = rows * 32 + 64;
+    const int words = mma_scratch_bytes(rows) / 4;
     if ((off + words) * 4 > max_smem) return false;
     L.mma_off = off;
     L.mma_rows = rows;
@@ -122,8 +122,7 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
     bool tensor = false;
     if constexpr (MmaEnabled<T>::value) {
         if (L.mma_off >= 0) {
-            uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
-            mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
+            mma_init<T>(mcx, reinterpret_cast<uint8_t *>(smem + L.mma_off), L.mma_rows, L.mma_cols);
             tensor = true;
         } else {
             mma_decline();
@@ -372,21 +371,28 @@ int mpdiv_imad_probe(uint32_t *sink, int kind, int iters, unsigned long long *pr
 // tensor-core issue-rate probe (include/mpdiv.h: mpdiv_mma_probe)
 // ---------------------------------------------------------------------------------------
 // One block of 128 threads per SM; `issuers` warps (1 or 2) each issue `iters` steps of four
-// tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols, A in tensor memory, B = swizzled shared-memory rows) into
-// their own accumulator columns, in the warp form the multiplier uses (mp_mma.cuh: operand words in ordinary
-// registers, one lane elected around the four MMAs and the commit).  Operand contents are arbitrary; nothing
-// is read back.  cycles[warp] of block 0 = clock64 from the first issue to the completion barrier.
+// tcgen05.mma.kind::i8 (M = 128, K = 32, N = n_cols, B = swizzled shared-memory rows) into their own accumulator
+// columns, in the warp form the multiplier uses (mp_mma.cuh: operand words in ordinary registers, one lane elected
+// around the four MMAs and the commit).  form 0: A in tensor memory (the pure rate of the pipe: the roofline
+// denominator); form 1: A read from shared memory through the overlapped Toeplitz descriptor, as the multiplier
+// issues it.  Operand contents are arbitrary; nothing is read back.  cycles[warp] of block 0 = clock64 from the
+// first issue to the completion barrier.
+}  // extern "C"
 constexpr int MMA_PROBE_ROWS = 272;
+template <int FORM>
 __global__ void __launch_bounds__(128)
 mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
 {
     extern __shared__ __align__(1024) uint8_t psm[];
-    uint8_t *brows = psm, *bars = psm + MMA_PROBE_ROWS * 128;
-    for (int i = threadIdx.x; i < MMA_PROBE_ROWS * 32; i += 128) reinterpret_cast<uint32_t *>(psm)[i] = (uint32_t)i * 2654435761u;
+    for (int i = threadIdx.x; i < mma_scratch_bytes(MMA_PROBE_ROWS) / 4 - 64; i += 128)
+        reinterpret_cast<uint32_t *>(psm)[i] = (uint32_t)i * 2654435761u;
     MmaCtx cx;
-    mma_init<128>(cx, brows, MMA_PROBE_ROWS, bars, 512);
+    mma_init<128>(cx, psm, MMA_PROBE_ROWS, 512);
     if (threadIdx.x == 0) {
-        mbar_init(cx.bar + 136, 1);                      // completion barrier of the second issuer
+        mbar_init(cx.bar + 192, 1);                      // the probe's own barriers: one completion barrier and one
+        mbar_init(cx.bar + 200, 1);                      // per-step commit target per issuer (nobody waits on those)
+        mbar_init(cx.bar + 208, 1);
+        mbar_init(cx.bar + 216, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     fence_async_smem();
@@ -397,24 +403,36 @@ mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
         const uint32_t idesc0 = mma_idesc(n_cols);
         for (int it = 0; it < iters; ++it) {
             uint32_t d_tmem = cx.tmem_base + 128u * (uint32_t)warp, a_tmem = cx.tmem_base + 256u + 32u * (uint32_t)(it & 3);
-            uint32_t b_lo = mma_desc_lo(smem_u32(brows + (it & 7) * 128)), idesc = idesc0, ebar = cx.bar + 64 + 8 * warp;
-            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(b_lo), "+r"(idesc), "+r"(ebar));
-            if (elect_one()) {
-                tc_mma_i8_ts_lo(d_tmem, a_tmem, b_lo, idesc, 1u);
-                tc_mma_i8_ts_lo(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
-                tc_mma_i8_ts_lo(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
-                tc_mma_i8_ts_lo(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
-                tc_commit(ebar);
+            uint32_t a_lo = mma_desc_lo(smem_u32(cx.ring) + 128u * (uint32_t)(it % RING_SEGS));
+            uint32_t b_lo = mma_desc_lo(smem_u32(cx.brows + (it & 7) * 128)), idesc = idesc0, ebar = cx.bar + 208 + 8 * warp;
+            asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(a_lo), "+r"(b_lo), "+r"(idesc), "+r"(ebar));
+            if (FORM == 0) {
+                if (elect_one()) {
+                    tc_mma_i8_ts(d_tmem, a_tmem, b_lo, idesc, 1u);
+                    tc_mma_i8_ts(d_tmem, a_tmem + 8, b_lo + 2, idesc, 1u);
+                    tc_mma_i8_ts(d_tmem, a_tmem + 16, b_lo + 4, idesc, 1u);
+                    tc_mma_i8_ts(d_tmem, a_tmem + 24, b_lo + 6, idesc, 1u);
+                    tc_commit(ebar);
+                }
+            } else {
+                if (elect_one()) {
+                    tc_mma_i8_ss(d_tmem, a_lo, b_lo, idesc, 1u);
+                    tc_mma_i8_ss(d_tmem, a_lo + 2, b_lo + 2, idesc, 1u);
+                    tc_mma_i8_ss(d_tmem, a_lo + 4, b_lo + 4, idesc, 1u);
+                    tc_mma_i8_ss(d_tmem, a_lo + 6, b_lo + 6, idesc, 1u);
+                    tc_commit(ebar);
+                }
             }
         }
-        if (elect_one()) tc_commit(cx.bar + 128 + 8 * warp);
+        if (elect_one()) tc_commit(cx.bar + 192 + 8 * warp);
         __syncwarp();
-        const bool ok = mbar_wait(cx.bar + 128 + 8 * warp, 0);
+        const bool ok = mbar_wait(cx.bar + 192 + 8 * warp, 0);
         const long long t1 = clock64();
         if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) cycles[warp] = ok ? (unsigned long long)(t1 - t0) : 0ull;
     }
     mma_fini<128>(cx);
 }
+extern "C" {
 
 unsigned long long mpdiv_mma_probe_macs(int n_cols, int issuers, int iters)
 {
@@ -423,14 +441,16 @@ unsigned long long mpdiv_mma_probe_macs(int n_cols, int issuers, int iters)
     return (unsigned long long)g_sm_count * issuers * iters * 4ull * 128ull * (unsigned long long)n_cols * 32ull;
 }
 
-int mpdiv_mma_probe(int n_cols, int issuers, int iters, unsigned long long *cycles, mpdiv_stream_t stream)
+int mpdiv_mma_probe(int n_cols, int issuers, int iters, int form, unsigned long long *cycles, mpdiv_stream_t stream)
 {
-    if (!cycles || iters <= 0 || (issuers != 1 && issuers != 2) || n_cols < 16 || n_cols > 128 || (n_cols & 15))
+    if (!cycles || iters <= 0 || (issuers != 1 && issuers != 2) || n_cols < 16 || n_cols > 128 || (n_cols & 15) ||
+        (form != 0 && form != 1))
         return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
-    const int bytes = MMA_PROBE_ROWS * 128 + 1024;
-    if (set_smem(mma_probe_kernel, (size_t)bytes) != MPDIV_OK) return MPDIV_ERR_CUDA;
-    mma_probe_kernel<<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
+    const int bytes = mma_scratch_bytes(MMA_PROBE_ROWS);
+    if (set_smem(form ? mma_probe_kernel<1> : mma_probe_kernel<0>, (size_t)bytes) != MPDIV_OK) return MPDIV_ERR_CUDA;
+    if (form) mma_probe_kernel<1><<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
+    else mma_probe_kernel<0><<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
     return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 

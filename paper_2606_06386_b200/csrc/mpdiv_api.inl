@@ -48,17 +48,18 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
     return L;
 }
 
-// Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the ring of
-// row operand (output blocks + steps rows of 128 bytes) and the mbarriers; the Toeplitz tiles live in tensor
-// memory.  max_smem in bytes.
-static void div_layout_add_mma(DivLayout &L, int M, int max_smem, int stages)
+// Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the rows of the
+// row operand (output blocks + steps rows of 128 bytes), the ring of the Toeplitz operand and the mbarriers.
+// max_smem in bytes.
+static void div_layout_add_mma(DivLayout &L, int M, int max_smem)
 {
     const int blocks = (M / 2 + 1 + 9 + 31) / 32 + 2;             // output blocks of u * shinv at n = M/2
-    const int need = ((blocks + 15) & ~15) + stages * MMA_STAGE_COLS;  // accumulators + the Toeplitz stages
-    const int cols = need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
-    const int rows = round_up(((blocks + 15) & ~15) + blocks + 8, 8);
+    const int nn = (blocks + 15) & ~15;
+    const int want = 2 * nn;                                      // one accumulator set per issuing warp (mp_mma.cuh)
+    const int cols = want <= 32 ? 32 : want <= 64 ? 64 : want <= 128 ? 128 : want <= 256 ? 256 : 512;
+    const int rows = round_up(nn + blocks, 8);
     const int off = round_up(L.total_words, 256);
-    const int words = rows * 32 + 64;
+    const int words = mma_scratch_bytes(rows) / 4;
     if ((off + words) * 4 > max_smem) return;
     L.mma_off = off;
     L.mma_rows = rows;
@@ -228,8 +229,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     MmaCtx *mma = nullptr;
     if constexpr (MMA) {
         if (L.mma_off >= 0 && clip) {
-            uint8_t *base = reinterpret_cast<uint8_t *>(smem + L.mma_off);
-            mma_init<T>(mcx, base, L.mma_rows, base + L.mma_rows * 128, L.mma_cols);
+            mma_init<T>(mcx, reinterpret_cast<uint8_t *>(smem + L.mma_off), L.mma_rows, L.mma_cols);
             mma = &mcx;
         } else {
             mma_decline();
@@ -448,11 +448,6 @@ namespace {
 
 std::mutex g_host_call_mutex;          // serialises mpdiv_batch_host's enqueue (its calls share events)
 
-template <int T, bool E = MmaEnabled<T>::value>
-struct MmaStagesOf { static constexpr int value = 0; };
-template <int T>
-struct MmaStagesOf<T, true> { static constexpr int value = MmaRoles<T>::STAGES; };
-
 // Early Newton iterations (l <= 33) run on warp 0 alone when the SMs hold several blocks each: the idle warps
 // give their issue slots to the other blocks.  A batch that leaves SMs with a single block is latency bound.
 // low byte: l up to which Refine runs on warp 0 alone; bit 8: MPDIV_NO_SEED (tuning: start Refine at l = 2)
@@ -492,7 +487,7 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
                  cudaStream_t st, int clip, int sched, bool tensor, const Tune &tn)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    if (MMA && tensor) div_layout_add_mma(L, u_limbs, g_max_smem, MmaStagesOf<T>::value);
+    if (MMA && tensor) div_layout_add_mma(L, u_limbs, g_max_smem);
     const size_t bytes = (size_t)L.total_words * 4;
     int rc = set_smem(mpdiv_kernel<T, LAT, MMA>, bytes);
     if (rc != MPDIV_OK) return rc;
