@@ -21,7 +21,7 @@
 //     unit, so with LBO = 16 bytes (core matrices that OVERLAP) the whole group is one reversed string
 //     C_g[y] = a[128 p + g + 112 - y], y < 240, read at unit r + c for K-chunk c; the 16 groups are the same
 //     string shifted by one byte each, 16 copies SBO bytes apart.  Consecutive steps slide the window by 128
-//     bytes, so a step costs 16 x 128 new bytes (one 16-byte store per producer thread) in a ring of RING_SEGS
+//     bytes, so a step costs 16 x 128 new bytes (one 16-byte store per producer thread) in a ring of four or six
 //     128-byte segments per copy (plus a mirror of segment 0 that keeps every window contiguous) -- against
 //     16 KB per step when the tile was generated row by row into tensor memory (33 LDS + 32 PRMT + a 32-register
 //     tcgen05.st per thread and step: ~330 cycles per step whatever N was, the limit of round 1).
@@ -51,13 +51,16 @@ namespace mpd {
 constexpr uint32_t MMA_SPIN_LIMIT = 1u << MMA_SPIN_LIMIT_LOG2;
 
 // shared-memory scratch of the engine: rows of the row operand | ring of the Toeplitz operand | mbarriers
-constexpr int RING_PAIRS = 3;                              // the ring is recycled in pairs of segments (see the issuers)
-constexpr int RING_SEGS = 2 * RING_PAIRS;                  // 128-byte segments per copy (+ 1 mirror of segment 0)
+// The ring is recycled in pairs of segments (see the issuers): three pairs, two in 128-thread blocks (four of them
+// share an SM's shared memory).
+__host__ __device__ constexpr int ring_pairs(int T) { return T <= 128 ? 2 : 3; }
+__host__ __device__ constexpr int ring_segs(int T) { return 2 * ring_pairs(T); }              // 128-byte segments per copy
+__host__ __device__ constexpr int ring_copy_bytes(int T) { return (ring_segs(T) + 1) * 128; }   // + 1 mirror of segment 0; = SBO
+__host__ __device__ constexpr int ring_bytes(int T) { return 16 * ring_copy_bytes(T); }
 constexpr int MMA_ISSUERS = 2;                             // issuing warps, one accumulator set each
-constexpr int RING_COPY_BYTES = (RING_SEGS + 1) * 128;     // = SBO of the Toeplitz descriptor
-constexpr int RING_BYTES = 16 * RING_COPY_BYTES;
 constexpr int MMA_BAR_BYTES = 256;                         // full[s] +8s, empty[pair] +64+8 pair, done +128, TMEM slot +160
-__host__ __device__ constexpr int mma_scratch_bytes(int rows) { return rows * 128 + RING_BYTES + MMA_BAR_BYTES; }
+// rows of the row operand | ring of the Toeplitz operand (the mbarriers live elsewhere: MMA_BAR_BYTES of their own)
+__host__ __device__ constexpr int mma_scratch_bytes(int rows, int T) { return rows * 128 + ring_bytes(T); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
@@ -98,9 +101,9 @@ __device__ __forceinline__ void tc_commit(uint32_t bar)
 
 // Shared-memory matrix descriptors, given by their low words; the high words are constants.
 //   row operand  : K-major SWIZZLE_128B, rows of 128 bytes, 8-row groups 1024 bytes apart
-//   Toeplitz     : K-major no swizzle, LBO = 16 bytes (overlapping core matrices), SBO = RING_COPY_BYTES
+//   Toeplitz     : K-major no swizzle, LBO = 16 bytes (overlapping core matrices), SBO = ring_copy_bytes(T)
 constexpr uint32_t DESC_HI_ROWS = (1024u >> 4) | (1u << 14) | (2u << 29);
-constexpr uint32_t DESC_HI_RING = ((uint32_t)RING_COPY_BYTES >> 4) | (1u << 14);
+__host__ __device__ constexpr uint32_t desc_hi_ring(int T) { return ((uint32_t)ring_copy_bytes(T) >> 4) | (1u << 14); }
 __device__ __forceinline__ uint32_t mma_desc_lo(uint32_t saddr) { return ((saddr >> 4) & 0x3FFFu) | (1u << 16); }
 __device__ __forceinline__ uint32_t mma_idesc(int n_cols)      // u8 x u8 -> s32, both K-major, M = 128
 {
@@ -109,9 +112,11 @@ __device__ __forceinline__ uint32_t mma_idesc(int n_cols)      // u8 x u8 -> s32
 // D[tmem] (+)= A[smem, Toeplitz descriptor] x B[smem, row descriptor], u8 x u8 -> s32, M = 128, K = 32.
 // The issuer prepares the words in ordinary registers BEFORE it elects its lane, so that the elected path is
 // R2UR + tcgen05.mma only (arithmetic on the uniform datapath sits on the issue path).
+template <int T>
 __device__ __forceinline__ void tc_mma_i8_ss(uint32_t tmem_d, uint32_t adesc_lo, uint32_t bdesc_lo, uint32_t idesc,
                                              uint32_t accumulate)
 {
+    constexpr uint32_t DESC_HI_RING = desc_hi_ring(T);
     const uint32_t z = 0;
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 ad, bd;\n\tsetp.ne.b32 p, %4, 0;\n\tmov.b64 ad, {%1, %6};\n\tmov.b64 bd, {%2, %7};\n\t"
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], ad, bd, %3, {%5, %5, %5, %5}, p;\n\t}"
@@ -159,18 +164,19 @@ struct MmaRoles {
     static constexpr int WARPS = T / 32;
     static constexpr int FIRST_ISSUER = WARPS - MMA_ISSUERS;
     static constexpr int PRODUCERS = WARPS == 4 ? 2 : 4;
+    static constexpr int RING_PAIRS = ring_pairs(T), RING_SEGS = ring_segs(T), RING_COPY_BYTES = ring_copy_bytes(T);
     static_assert(WARPS >= 4 && RING_SEGS <= 8 && RING_PAIRS <= 4 && MMA_ISSUERS == 2, "128 threads or more, two issuers");
 };
 
 // One-time setup per block: mbarriers, TMEM allocation (warp 0 owns it).  All threads call it.
-// scratch: mma_scratch_bytes(rows) bytes, 1024-byte aligned.
+// scratch: mma_scratch_bytes(rows, T) bytes, 1024-byte aligned (rewritten by every product: it may overlap buffers
+// that are dead while a product runs); bars: MMA_BAR_BYTES that nothing else ever touches.
 template <int T>
-__device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *scratch, int rows, int tmem_cols)
+__device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *scratch, int rows, uint8_t *bars, int tmem_cols)
 {
     cx.brows = scratch;
     cx.brows_cap = rows;
     cx.ring = scratch + rows * 128;
-    uint8_t *bars = cx.ring + RING_BYTES;
     cx.bar = smem_u32(bars);
     cx.tmem_cols = tmem_cols;
     cx.ndone = 0;
@@ -179,8 +185,8 @@ __device__ __forceinline__ void mma_init(MmaCtx &cx, uint8_t *scratch, int rows,
     cx.empty_par = 0;
     uint32_t *slot = reinterpret_cast<uint32_t *>(bars + 160);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < RING_SEGS; s++) mbar_init(cx.bar + 8 * s, 1);                    // the segment's producer warp
-        for (int s = 0; s < RING_PAIRS; s++) mbar_init(cx.bar + 64 + 8 * s, 2);              // the commits of the pair's two steps
+        for (int s = 0; s < ring_segs(T); s++) mbar_init(cx.bar + 8 * s, 1);                 // the segment's producer warp
+        for (int s = 0; s < ring_pairs(T); s++) mbar_init(cx.bar + 64 + 8 * s, 2);           // the commits of the pair's two steps
         mbar_init(cx.bar + 128, MMA_ISSUERS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -284,6 +290,7 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
                                           limb *P, limb *HI, Blk &blk)
 {
     using Roles = MmaRoles<T>;
+    constexpr int RING_PAIRS = Roles::RING_PAIRS, RING_SEGS = Roles::RING_SEGS, RING_COPY_BYTES = Roles::RING_COPY_BYTES;
     MmaCtx cx = cx_mem;        // work on a register copy: the asm memory clobbers would reload every field
     const int tid = threadIdx.x, warp = tid >> 5;
     const int Ea = (na + 31) / 32, Eb = (nb + 31) / 32;
@@ -373,10 +380,10 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
                     uint32_t d_tmem = d_base, idesc = mma_idesc(Nn), ac = acc0;
                     asm volatile("" : "+r"(d_tmem), "+r"(a_lo), "+r"(b_lo), "+r"(idesc), "+r"(ac), "+r"(ebar));
                     if (elect_one()) {
-                        tc_mma_i8_ss(d_tmem, a_lo, b_lo, idesc, ac);
-                        tc_mma_i8_ss(d_tmem, a_lo + 2, b_lo + 2, idesc, 1u);
-                        tc_mma_i8_ss(d_tmem, a_lo + 4, b_lo + 4, idesc, 1u);
-                        tc_mma_i8_ss(d_tmem, a_lo + 6, b_lo + 6, idesc, 1u);
+                        tc_mma_i8_ss<T>(d_tmem, a_lo, b_lo, idesc, ac);
+                        tc_mma_i8_ss<T>(d_tmem, a_lo + 2, b_lo + 2, idesc, 1u);
+                        tc_mma_i8_ss<T>(d_tmem, a_lo + 4, b_lo + 4, idesc, 1u);
+                        tc_mma_i8_ss<T>(d_tmem, a_lo + 6, b_lo + 6, idesc, 1u);
                         tc_commit(ebar);
                     }
                 } else {
@@ -387,10 +394,10 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
                         uint32_t bl = b_lo + 8u * (uint32_t)nc, al = a_lo, ac = acc0;
                         asm volatile("" : "+r"(d_tmem), "+r"(al), "+r"(bl), "+r"(idesc), "+r"(ac));
                         if (elect_one()) {
-                            tc_mma_i8_ss(d_tmem, al, bl, idesc, ac);
-                            tc_mma_i8_ss(d_tmem, al + 2, bl + 2, idesc, 1u);
-                            tc_mma_i8_ss(d_tmem, al + 4, bl + 4, idesc, 1u);
-                            tc_mma_i8_ss(d_tmem, al + 6, bl + 6, idesc, 1u);
+                            tc_mma_i8_ss<T>(d_tmem, al, bl, idesc, ac);
+                            tc_mma_i8_ss<T>(d_tmem, al + 2, bl + 2, idesc, 1u);
+                            tc_mma_i8_ss<T>(d_tmem, al + 4, bl + 4, idesc, 1u);
+                            tc_mma_i8_ss<T>(d_tmem, al + 6, bl + 6, idesc, 1u);
                         }
                     }
                     if (elect_one()) tc_commit(ebar);

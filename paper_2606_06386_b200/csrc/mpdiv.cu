@@ -100,7 +100,7 @@ static bool mul_layout_add_mma(MulLayout &L, int a_limbs, int b_limbs, int c_lim
         L.total_words = o;
     }
     const int off = round_up(L.total_words, 256);
-    const int words = mma_scratch_bytes(rows) / 4;
+    const int words = (mma_scratch_bytes(rows, 512) + MMA_BAR_BYTES) / 4;     // launch_mul<512> runs this engine
     if ((off + words) * 4 > max_smem) return false;
     L.mma_off = off;
     L.mma_rows = rows;
@@ -122,7 +122,8 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
     bool tensor = false;
     if constexpr (MmaEnabled<T>::value) {
         if (L.mma_off >= 0) {
-            mma_init<T>(mcx, reinterpret_cast<uint8_t *>(smem + L.mma_off), L.mma_rows, L.mma_cols);
+            uint8_t *scratch = reinterpret_cast<uint8_t *>(smem + L.mma_off);
+            mma_init<T>(mcx, scratch, L.mma_rows, scratch + mma_scratch_bytes(L.mma_rows, T), L.mma_cols);
             tensor = true;
         } else {
             mma_decline();
@@ -384,10 +385,10 @@ __global__ void __launch_bounds__(128)
 mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
 {
     extern __shared__ __align__(1024) uint8_t psm[];
-    for (int i = threadIdx.x; i < mma_scratch_bytes(MMA_PROBE_ROWS) / 4 - 64; i += 128)
+    for (int i = threadIdx.x; i < mma_scratch_bytes(MMA_PROBE_ROWS, 128) / 4; i += 128)
         reinterpret_cast<uint32_t *>(psm)[i] = (uint32_t)i * 2654435761u;
     MmaCtx cx;
-    mma_init<128>(cx, psm, MMA_PROBE_ROWS, 512);
+    mma_init<128>(cx, psm, MMA_PROBE_ROWS, psm + mma_scratch_bytes(MMA_PROBE_ROWS, 128), 512);
     if (threadIdx.x == 0) {
         mbar_init(cx.bar + 192, 1);                      // the probe's own barriers: one completion barrier and one
         mbar_init(cx.bar + 200, 1);                      // per-step commit target per issuer (nobody waits on those)
@@ -403,7 +404,7 @@ mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
         const uint32_t idesc0 = mma_idesc(n_cols);
         for (int it = 0; it < iters; ++it) {
             uint32_t d_tmem = cx.tmem_base + 128u * (uint32_t)warp, a_tmem = cx.tmem_base + 256u + 32u * (uint32_t)(it & 3);
-            uint32_t a_lo = mma_desc_lo(smem_u32(cx.ring) + 128u * (uint32_t)(it % RING_SEGS));
+            uint32_t a_lo = mma_desc_lo(smem_u32(cx.ring) + 128u * (uint32_t)(it % ring_segs(128)));
             uint32_t b_lo = mma_desc_lo(smem_u32(cx.brows + (it & 7) * 128)), idesc = idesc0, ebar = cx.bar + 208 + 8 * warp;
             asm volatile("" : "+r"(d_tmem), "+r"(a_tmem), "+r"(a_lo), "+r"(b_lo), "+r"(idesc), "+r"(ebar));
             if (FORM == 0) {
@@ -416,10 +417,10 @@ mma_probe_kernel(int n_cols, int issuers, int iters, unsigned long long *cycles)
                 }
             } else {
                 if (elect_one()) {
-                    tc_mma_i8_ss(d_tmem, a_lo, b_lo, idesc, 1u);
-                    tc_mma_i8_ss(d_tmem, a_lo + 2, b_lo + 2, idesc, 1u);
-                    tc_mma_i8_ss(d_tmem, a_lo + 4, b_lo + 4, idesc, 1u);
-                    tc_mma_i8_ss(d_tmem, a_lo + 6, b_lo + 6, idesc, 1u);
+                    tc_mma_i8_ss<128>(d_tmem, a_lo, b_lo, idesc, 1u);
+                    tc_mma_i8_ss<128>(d_tmem, a_lo + 2, b_lo + 2, idesc, 1u);
+                    tc_mma_i8_ss<128>(d_tmem, a_lo + 4, b_lo + 4, idesc, 1u);
+                    tc_mma_i8_ss<128>(d_tmem, a_lo + 6, b_lo + 6, idesc, 1u);
                     tc_commit(ebar);
                 }
             }
@@ -447,7 +448,7 @@ int mpdiv_mma_probe(int n_cols, int issuers, int iters, int form, unsigned long 
         (form != 0 && form != 1))
         return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
-    const int bytes = mma_scratch_bytes(MMA_PROBE_ROWS);
+    const int bytes = mma_scratch_bytes(MMA_PROBE_ROWS, 128) + MMA_BAR_BYTES;
     if (set_smem(form ? mma_probe_kernel<1> : mma_probe_kernel<0>, (size_t)bytes) != MPDIV_OK) return MPDIV_ERR_CUDA;
     if (form) mma_probe_kernel<1><<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);
     else mma_probe_kernel<0><<<g_sm_count, 128, bytes, reinterpret_cast<cudaStream_t>(stream)>>>(n_cols, issuers, iters, cycles);

@@ -7,26 +7,34 @@
 // ---------------------------------------------------------------------------------------
 struct DivLayout {
     int v_off, u_off, wa_off, big_off, sc_off, total_words;
-    int mma_off;      // word offset (1024-byte aligned) of the tensor-core scratch, or -1: rows | barriers
+    int mma_off;      // word offset (1024-byte aligned) of the tensor-core scratch (rows | ring), or -1
+    int bar_off;      // word offset of the engine's mbarriers (MMA_BAR_BYTES that no buffer of either layout overlaps)
     int mma_rows;     // rows of 128 bytes available for the row operand
     int mma_cols;     // TMEM columns to allocate
     int x_words;      // Refine: X at big_off, P behind it
     int p_words_r;    // Refine: capacity of P and of HI
     int p_words_q;    // quotient phase: capacity of P and of HI
+    int hcap;         // the layout holds instances with H = max(h - k, 2) <= hcap
 };
 
 // M: limbs of the dividend side (u stride, or h for shinv_batch); n: divisor stride;
 // with_quotient: reserve the product scratch of u * shinv and v * q; clip: MPDIV_VARIANT_CLIPPED, whose
 // products only store the limbs they keep (about M/2 in Refine, M in the quotient phase).
-static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
+// hcap: 0 = any instance of these strides (H up to M: a short divisor has a long inverse and a long quotient);
+// otherwise the COMPACT layout for instances with H <= hcap: the iterate / quotient buffer WA and the quotient-phase
+// product shrink to what such instances need -- at the configs' shape (H = M/2 + 1) that is 8 KB of 40 at
+// 2^16 bits, the room the tensor-core scratch needs to keep four blocks on an SM.  V, U and the block scratch sit
+// at the same offsets in both layouts, so the operands are loaded before the layout of the instance is known.
+static DivLayout div_layout(int M, int n, bool with_quotient, bool clip, int hcap = 0)
 {
     DivLayout L;
     const int Mp = round_up(M, TILE);
     const int np = round_up(n, TILE);
+    const int hc = (hcap > 0 && hcap < Mp) ? round_up(hcap, TILE) : Mp;
     if (clip) {
         L.x_words = round_up(Mp / 2 + 96, TILE);
         L.p_words_r = round_up(Mp / 2 + 160, TILE);
-        L.p_words_q = with_quotient ? (Mp > np ? Mp : np) + 64 : 0;
+        L.p_words_q = with_quotient ? (hc > np ? hc : np) + 104 : 0;
     } else {
         L.x_words = np + 48;
         L.p_words_r = Mp + 48;
@@ -36,35 +44,71 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip)
     const int big_r = L.x_words + 2 * L.p_words_r + 2 * ovr;
     const int big_q = 2 * L.p_words_q + 2 * ovq;
     int o = 0;
+    L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
     L.v_off = o; o += np + 16;
     L.u_off = o; o += Mp + 16;
-    L.wa_off = o; o += Mp + 16;
+    L.wa_off = o; o += hc + 24;
     L.big_off = o; o += (big_r > big_q ? big_r : big_q);
-    L.sc_off = o; o += (int)(sizeof(BlkScratch) / 4);
     L.total_words = o;
     L.mma_off = -1;
+    L.bar_off = -1;
     L.mma_rows = 0;
     L.mma_cols = 0;
+    L.hcap = hc;
     return L;
 }
 
-// Adds the scratch of the tensor-core multiplier (mp_mma.cuh) when the block has room for it: the rows of the
-// row operand (output blocks + steps rows of 128 bytes), the ring of the Toeplitz operand and the mbarriers.
-// max_smem in bytes.
-static void div_layout_add_mma(DivLayout &L, int M, int max_smem)
+// H up to which an instance takes the compact layout: the configs' shape H = M/2 + 1 with room to spare.
+static int compact_hcap(int M) { return round_up(M, TILE) / 2 + 40; }
+
+// Places the scratch of the tensor-core multiplier (mp_mma.cuh) behind layout Lx: the rows of the row operand (output
+// blocks + steps rows of 128 bytes) and the ring of the Toeplitz operand.  Returns the word offset where the scratch
+// ends, or -1 (and leaves Lx without an engine) when that would pass limit_words.  threads = block size.
+static int div_layout_place_mma(DivLayout &Lx, int M, int limit_words, int threads)
 {
     const int blocks = (M / 2 + 1 + 9 + 31) / 32 + 2;             // output blocks of u * shinv at n = M/2
     const int nn = (blocks + 15) & ~15;
     const int want = 2 * nn;                                      // one accumulator set per issuing warp (mp_mma.cuh)
     const int cols = want <= 32 ? 32 : want <= 64 ? 64 : want <= 128 ? 128 : want <= 256 ? 256 : 512;
     const int rows = round_up(nn + blocks, 8);
-    const int off = round_up(L.total_words, 256);
-    const int words = mma_scratch_bytes(rows) / 4;
-    if ((off + words) * 4 > max_smem) return;
-    L.mma_off = off;
-    L.mma_rows = rows;
-    L.mma_cols = cols;
-    L.total_words = off + words;
+    const int off = round_up(Lx.total_words, 256);
+    const int end = off + mma_scratch_bytes(rows, threads) / 4;
+    if (end > limit_words) return -1;
+    Lx.mma_off = off;
+    Lx.mma_rows = rows;
+    Lx.mma_cols = cols;
+    return end;
+}
+
+// The two layouts of a division kernel that carries the engine, and the bytes to allocate.
+//   Lc  compact layout (instances with H <= Lc.hcap) + scratch: the common case, and the fastest arrangement
+//   Lf  full layout (any instance); it gets a scratch of its own behind it when that still keeps per_sm blocks on an
+//       SM (2^17 bits and up), otherwise its instances run without the engine and may overrun Lc's scratch, which every
+//       product rewrites.  The mbarriers sit behind everything (Lc.bar_off == Lf.bar_off).
+static size_t div_layouts_with_mma(DivLayout &Lf, DivLayout &Lc, int u_limbs, int v_limbs, bool clip, int threads, int per_sm,
+                                   int max_smem)
+{
+    Lf = div_layout(u_limbs + 1, v_limbs, true, clip);
+    Lc = div_layout(u_limbs + 1, v_limbs, true, clip, compact_hcap(u_limbs + 1));
+    const int bar_words = MMA_BAR_BYTES / 4;
+    const int budget = (max_smem + 1024) / per_sm - 1024;        // shared memory of an SM = the per-block maximum + 1 KB
+    int limit = (budget < max_smem ? budget : max_smem) / 4 - bar_words;
+    int end_c = div_layout_place_mma(Lc, u_limbs, limit, threads);
+    if (end_c < 0) {                                             // give up occupancy before giving up the engine
+        limit = max_smem / 4 - bar_words;
+        end_c = div_layout_place_mma(Lc, u_limbs, limit, threads);
+    }
+    int end = Lf.total_words;
+    if (end_c >= 0) {
+        if (end_c > end) end = end_c;
+        const int end_f = div_layout_place_mma(Lf, u_limbs, limit, threads);
+        if (end_f > end) end = end_f;
+        end = round_up(end, 4);
+        Lc.bar_off = Lf.bar_off = end;
+        end += bar_words;
+    }
+    Lc.total_words = Lf.total_words = end;
+    return (size_t)end * 4;
 }
 
 __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout &L)
@@ -208,28 +252,24 @@ struct DivMma { static constexpr bool value = MmaEnabled<T>::value && !(LAT && T
 template <int T, bool LAT, bool MMA>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
-             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, int clip, int narrow_l,
+             limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, DivLayout Lc, int clip, int narrow_l,
              const limb *__restrict__ wmid)
 {
+    // L: the layout for any instance of these strides; Lc: the compact layout (H <= Lc.hcap); each with the tensor-core
+    // scratch behind it or mma_off < 0 (div_layouts_with_mma).  V, U and the block scratch coincide.
     extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
     limb *U = smem + L.u_off;          // dividend at U + 4 (same)
     limb *WA = smem + L.wa_off;        // shinv, then the quotient
     Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
-    const ShinvBufs rb = refine_bufs(smem, L);
-    // quotient-phase product scratch
-    limb *PQ = smem + L.big_off;
-    MulScratch mq;
-    mq.HI = PQ + L.p_words_q;
-    mq.OV = mq.HI + L.p_words_q;
-    mq.C3 = mq.OV + round_up(L.p_words_q / TILE, 4);
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
     static_assert(!MMA || DivMma<T, LAT>::value, "no tensor-core engine for this block size");
     MmaCtx mcx;
     MmaCtx *mma = nullptr;
     if constexpr (MMA) {
-        if (L.mma_off >= 0 && clip) {
-            mma_init<T>(mcx, reinterpret_cast<uint8_t *>(smem + L.mma_off), L.mma_rows, L.mma_cols);
+        if (Lc.mma_off >= 0 && clip) {
+            mma_init<T>(mcx, reinterpret_cast<uint8_t *>(smem + Lc.mma_off), Lc.mma_rows,
+                        reinterpret_cast<uint8_t *>(smem + Lc.bar_off), Lc.mma_cols);
             mma = &mcx;
         } else {
             mma_decline();
@@ -277,8 +317,25 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             Vb = V; k = 1; h = h + 1;
         }
 
+        // the layout of this instance: compact (and with it the tensor-core engine) when its inverse and quotient are
+        // short enough, the full one otherwise
+        const bool compact = mma != nullptr && max(h - k, 2) <= Lc.hcap;
+        const DivLayout &Li = compact ? Lc : L;
+        MmaCtx *mma_i = (mma != nullptr && Li.mma_off >= 0) ? mma : nullptr;
+        if (mma_i) {                                       // the scratch of this instance's layout
+            mcx.brows = reinterpret_cast<uint8_t *>(smem + Li.mma_off);
+            mcx.ring = mcx.brows + Li.mma_rows * 128;
+            mcx.brows_cap = Li.mma_rows;
+        }
+        const ShinvBufs rb = refine_bufs(smem, Li);
+        limb *PQ = smem + Li.big_off;      // quotient-phase product scratch
+        MulScratch mq;
+        mq.HI = PQ + Li.p_words_q;
+        mq.OV = mq.HI + Li.p_words_q;
+        mq.C3 = mq.OV + round_up(Li.p_words_q / TILE, 4);
+
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
-        const int nw = shinv_block<T, MMA>(Vb, k, h, rb, blk, clip != 0, mma, narrow_l & 255, !(narrow_l & 256),
+        const int nw = shinv_block<T, MMA>(Vb, k, h, rb, blk, clip != 0, mma_i, narrow_l & 255, !(narrow_l & 256),
                                       (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
 
@@ -330,7 +387,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 lin_zero<T>(Q, qlen);
             } else {
                 const int dlo = (h - 1) / 32;              // tensor-core form: E < B^(32 dlo + 1) <= B^h
-                int pl = try_mma_range<T, MMA>(mma, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
+                int pl = try_mma_range<T, MMA>(mma_i, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
                 if (pl >= 0) {
                     count(CNT_MMA_PRODUCTS);
                     lin_copy<T>(Q, qlen, PQ, pl, h - 32 * dlo);
@@ -346,7 +403,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             rlen = round_up(k + 3, TILE);
             int pl = 0;
             if (pq > 0) {
-                pl = try_mma_range<T, MMA>(mma, Vb, k + 1, Q, pq, 0, (rlen + 31) / 32, PQ, mq.HI, blk);
+                pl = try_mma_range<T, MMA>(mma_i, Vb, k + 1, Q, pq, 0, (rlen + 31) / 32, PQ, mq.HI, blk);
                 if (pl >= 0) {
                     count(CNT_MMA_PRODUCTS);
                     pl = min(rlen, pl);
@@ -487,8 +544,9 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
                  cudaStream_t st, int clip, int sched, bool tensor, const Tune &tn)
 {
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
-    if (MMA && tensor) div_layout_add_mma(L, u_limbs, g_max_smem);
-    const size_t bytes = (size_t)L.total_words * 4;
+    DivLayout Lc = L;                                        // Lc.mma_off < 0: no engine, Lc unused
+    size_t bytes = (size_t)L.total_words * 4;
+    if (MMA && tensor) bytes = div_layouts_with_mma(L, Lc, u_limbs, v_limbs, clip != 0, T, LAT ? 1 : 512 / T, g_max_smem);
     int rc = set_smem(mpdiv_kernel<T, LAT, MMA>, bytes);
     if (rc != MPDIV_OK) return rc;
     // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
@@ -503,7 +561,7 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
             shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
         }
     }
-    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, clip, narrow_for(sched, tn), wmid);
+    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid);
     const bool ok = cudaGetLastError() == cudaSuccess;
     if (wmid) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
