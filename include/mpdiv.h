@@ -48,7 +48,8 @@ enum {
     MPDIV_OK = 0,
     MPDIV_ERR_BAD_ARG = 1,      /* null pointer, non-positive size, misaligned pointer or stride */
     MPDIV_ERR_UNSUPPORTED = 2,  /* stride above MPDIV_MAX_LIMBS, or shared memory budget exceeded */
-    MPDIV_ERR_CUDA = 3          /* a CUDA runtime call failed (launch, attribute, copy) */
+    MPDIV_ERR_CUDA = 3,         /* a CUDA runtime call failed (launch, attribute, copy) */
+    MPDIV_ERR_TOO_LARGE = 4     /* mpdiv_batch_noalloc: batch above MPDIV_NOALLOC_MAX_BATCH */
 };
 
 /*
@@ -69,6 +70,24 @@ enum {
  */
 int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                 uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
+
+/*
+ * mpdiv_batch for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): same inputs, outputs, exact results and default variant as mpdiv_batch, but the one
+ * scratch buffer of the path -- the rows through which the head-of-Refine kernel hands its iterates to the
+ * division kernel, which mpdiv_batch takes from a stream-ordered memory pool -- is a static device array inside
+ * the library: MPDIV_NOALLOC_MAX_BATCH x 272 limbs = 4.25 MiB that every GPU that loads the library holds until
+ * the process exits.  The call makes no cudaMalloc / cudaFree / pool call of any kind (its first use on a device
+ * looks the array's address up with cudaGetSymbolAddress and sets kernel attributes, host side only).
+ *   batch > MPDIV_NOALLOC_MAX_BATCH returns MPDIV_ERR_TOO_LARGE and enqueues nothing: split the batch.
+ *   ALL calls on a device share the one array: calls whose kernels may overlap on the GPU (different streams
+ *   without an ordering between them, or several host threads) RACE on it and give wrong quotients; calls on one
+ *   stream, or ordered by events, are safe.  The array keeps the last call's contents; nothing in it has to start
+ *   at zero (every row that is read was written by the same call).
+ */
+#define MPDIV_NOALLOC_MAX_BATCH 4096
+int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
+                        uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
 
 /*
  * Variants of the method; both return the same exact (q, r).

@@ -17,7 +17,8 @@ from . import build as _build
 _LIB = None
 _VOIDP = ctypes.c_void_p
 
-OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA = 0, 1, 2, 3
+OK, ERR_BAD_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_TOO_LARGE = 0, 1, 2, 3, 4
+NOALLOC_MAX_BATCH = 4096
 VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
 VARIANT_DEFAULT = VARIANT_CLIPPED
 # tuning switches OR-ed into the `flags` of the *_ex calls (include/mpdiv.h)
@@ -53,6 +54,8 @@ def lib() -> ctypes.CDLL:
         i, sz = ctypes.c_int, ctypes.c_size_t
         L.mpdiv_batch.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
         L.mpdiv_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, i, _VOIDP]
+        L.mpdiv_batch_noalloc.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, _VOIDP, i, _VOIDP]
+        L.mpdiv_batch_noalloc.restype = i
         L.shinv_batch_ex.argtypes = [_VOIDP, i, i, _VOIDP, i, i, i, _VOIDP]
         L.mplinop_batch.argtypes = [i, _VOIDP, i, _VOIDP, i, i, _VOIDP, i, _VOIDP, i, _VOIDP]
         L.mpmul_batch_ex.argtypes = [_VOIDP, i, _VOIDP, i, _VOIDP, i, i, i, _VOIDP]
@@ -82,7 +85,7 @@ def lib() -> ctypes.CDLL:
     return _LIB
 
 
-EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
+EXPORTS = ("mplinop_batch", "mpdiv_batch", "mpdiv_batch_ex", "mpdiv_batch_noalloc", "mpmul_batch", "mpmul_batch_ex", "shinv_batch", "shinv_batch_ex", "mpdiv_host_workspace_bytes",
            "mpdiv_batch_host", "mpdiv_imad_probe_threads", "mpdiv_imad_probe", "mpdiv_mma_probe", "mpdiv_mma_probe_macs",
            "mpdiv_debug_counters", "mpdiv_status", "mpdiv_seed_batch", "mpdiv_batch_launches", "mpdiv_version", "mpdiv_strerror")
 
@@ -139,6 +142,20 @@ def mpdiv_batch(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor | None = None,
     else:
         _raise(lib().mpdiv_batch_ex(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
                                     int(variant), _stream_ptr(stream)), "mpdiv_batch_ex")
+    return q, r
+
+
+def mpdiv_batch_noalloc(u: torch.Tensor, v: torch.Tensor, q: torch.Tensor, r: torch.Tensor, stream=None):
+    """mpdiv_batch through the entry point that allocates nothing (static scratch inside the library, batch <=
+    NOALLOC_MAX_BATCH); the caller passes every buffer.  Calls that overlap on the GPU race on the scratch."""
+    for t, name in ((u, "u"), (v, "v"), (q, "q"), (r, "r")):
+        _check_dev(t, name)
+    batch, ul = u.shape
+    vl = v.shape[1]
+    if v.shape[0] != batch or tuple(q.shape) != (batch, ul) or tuple(r.shape) != (batch, vl):
+        raise ValueError("v, q, r must be (batch, v_limbs), (batch, u_limbs), (batch, v_limbs)")
+    _raise(lib().mpdiv_batch_noalloc(u.data_ptr(), ul, v.data_ptr(), vl, q.data_ptr(), r.data_ptr(), batch,
+                                     _stream_ptr(stream)), "mpdiv_batch_noalloc")
     return q, r
 
 

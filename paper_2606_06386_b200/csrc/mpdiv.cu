@@ -253,6 +253,7 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 struct Tune {
     bool no_seed, no_head, no_mma, no_cluster;
     int threads;                                 // 0 = by size
+    limb *wmid_fixed;                            // mpdiv_batch_noalloc: the head kernel's rows live here (no pool allocation)
 };
 Tune tune_of(int flags)
 {
@@ -263,6 +264,7 @@ Tune tune_of(int flags)
     t.no_cluster = (flags & MPDIV_FLAG_NO_CLUSTER) != 0;
     const int c = (flags & MPDIV_FLAG_THREADS_MASK) >> 8;
     t.threads = c >= 1 && c <= 4 ? 32 << c : 0;
+    t.wmid_fixed = nullptr;
     return t;
 }
 bool flags_ok(int flags)
@@ -464,6 +466,7 @@ const char *mpdiv_strerror(int code)
         case MPDIV_ERR_BAD_ARG: return "bad argument (null pointer, non-positive size, misaligned pointer or stride)";
         case MPDIV_ERR_UNSUPPORTED: return "unsupported size (stride above MPDIV_MAX_LIMBS or shared memory budget exceeded)";
         case MPDIV_ERR_CUDA: return "CUDA runtime error";
+        case MPDIV_ERR_TOO_LARGE: return "batch larger than MPDIV_NOALLOC_MAX_BATCH: the static scratch of mpdiv_batch_noalloc holds no more";
         default: return "unknown status";
     }
 }
@@ -471,3 +474,48 @@ const char *mpdiv_strerror(int code)
 }  // extern "C"
 
 #include "mpdiv_api.inl"
+
+// ---------------------------------------------------------------------------------------
+// mpdiv_batch_noalloc (include/mpdiv.h): the division for callers that must not allocate
+// ---------------------------------------------------------------------------------------
+// The one scratch buffer of the division path is the workspace through which the head-of-Refine kernel hands its
+// iterates to the division kernel (batch x WMID_STRIDE limbs; mpdiv_batch takes it from a stream-ordered memory
+// pool).  Here it is a file-scope device array: every GPU that loads the library holds these
+// MPDIV_NOALLOC_MAX_BATCH x 272 x 4 bytes = 4.25 MiB until the process exits.  In host code the NAME of the array is
+// a host-side stand-in, not a device address: its device address is looked up once per device with
+// cudaGetSymbolAddress (that device current) and that pointer is what the kernels get.
+static __device__ __align__(256) limb g_noalloc_wmid[(size_t)MPDIV_NOALLOC_MAX_BATCH * WMID_STRIDE];
+
+namespace {
+limb *noalloc_scratch()
+{
+    static limb *ptr[MAX_DEVICES] = {nullptr};
+    std::lock_guard<std::mutex> lk(g_host_mutex);
+    if (!ptr[g_dev]) {                                       // g_dev: the current device, set by device_props()
+        void *p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_noalloc_wmid) != cudaSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        ptr[g_dev] = static_cast<limb *>(p);
+    }
+    return ptr[g_dev];
+}
+}  // namespace
+
+extern "C" int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
+                                   int batch, mpdiv_stream_t stream)
+{
+    int rc = check_div_args(u, u_limbs, v, v_limbs, q, r, batch);
+    if (rc != MPDIV_OK) return rc;
+    if (!aligned16(u) || !aligned16(v) || !aligned16(q) || !aligned16(r)) return MPDIV_ERR_BAD_ARG;
+    if (batch > MPDIV_NOALLOC_MAX_BATCH) return MPDIV_ERR_TOO_LARGE;       // the static scratch holds no more rows
+    if (!device_props()) return MPDIV_ERR_CUDA;
+    Tune tn = tune_of(MPDIV_VARIANT_DEFAULT);
+    tn.wmid_fixed = noalloc_scratch();
+    if (!tn.wmid_fixed) return MPDIV_ERR_CUDA;
+    // Nothing in the scratch has to start at zero: the head kernel writes the row of every instance whose row the
+    // division kernel reads (both derive that from the instance's precisions alone, mp_div.cuh head_plan), so what
+    // an earlier call left behind is never read.
+    return div_dispatch(u, u_limbs, v, v_limbs, q, r, batch, 1, reinterpret_cast<cudaStream_t>(stream), batch, tn);
+}

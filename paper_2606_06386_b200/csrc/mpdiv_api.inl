@@ -552,7 +552,10 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
     // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
     // iterate over in a stream-ordered workspace (mp_div.cuh "Head of Refine")
     limb *wmid = nullptr;
-    if (use_head(u_limbs, clip, LAT, tn)) {
+    if (use_head(u_limbs, clip, LAT, tn) && tn.wmid_fixed) {
+        wmid = tn.wmid_fixed;                                // mpdiv_batch_noalloc: the library's static scratch
+        shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
+    } else if (use_head(u_limbs, clip, LAT, tn)) {
         if (!head_pool() ||
             cudaMallocFromPoolAsync(reinterpret_cast<void **>(&wmid), (size_t)batch * WMID_STRIDE * sizeof(limb), head_pool(), st) != cudaSuccess) {
             cudaGetLastError();
@@ -563,7 +566,7 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
     }
     mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid);
     const bool ok = cudaGetLastError() == cudaSuccess;
-    if (wmid) cudaFreeAsync(wmid, st);
+    if (wmid && !tn.wmid_fixed) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
