@@ -26,8 +26,11 @@
  *     correction loop that hit its bound, v = 0) do not change the return value of the asynchronous
  *     call; they set sticky bits of a device status word that mpdiv_status() reads.  A caller that
  *     needs certainty polls it once per batch (tests do so after every batch; it must read 0).
- *   - Supported sizes: strides up to MPDIV_MAX_LIMBS limbs (2^18 bits, the paper's range,
- *     PAPER.md:194); any effective precision inside the stride, including 0.
+ *   - Supported sizes: operand strides up to MPDIV_MAX_OPERAND_LIMBS limbs (2^18 bits, the paper's range,
+ *     its ceiling is the shared memory of an SM); the DIVIDEND of mpdiv_batch may have up to
+ *     MPDIV_MAX_LIMBS limbs (2^19 bits: dividends above MPDIV_MAX_OPERAND_LIMBS limbs are not held on chip but
+ *     streamed from HBM window by window, see mpdiv_batch).  Any effective precision inside the stride,
+ *     including 0.
  */
 #ifndef MPDIV_H
 #define MPDIV_H
@@ -42,12 +45,14 @@ extern "C" {
 /* binary-compatible with cudaStream_t (0 / NULL = the legacy default stream) */
 typedef struct CUstream_st *mpdiv_stream_t;
 
-#define MPDIV_MAX_LIMBS 8192
+#define MPDIV_MAX_LIMBS 16384          /* u_limbs of mpdiv_batch (default variant) */
+#define MPDIV_MAX_OPERAND_LIMBS 8192   /* every other stride: v_limbs, h of shinv_batch, operands of mpmul_batch, and
+                                          u_limbs of MPDIV_VARIANT_PRINTED */
 
 enum {
     MPDIV_OK = 0,
     MPDIV_ERR_BAD_ARG = 1,      /* null pointer, non-positive size, misaligned pointer or stride */
-    MPDIV_ERR_UNSUPPORTED = 2,  /* stride above MPDIV_MAX_LIMBS, or shared memory budget exceeded */
+    MPDIV_ERR_UNSUPPORTED = 2,  /* stride above MPDIV_MAX_(OPERAND_)LIMBS, or shared memory budget exceeded */
     MPDIV_ERR_CUDA = 3,         /* a CUDA runtime call failed (launch, attribute, copy) */
     MPDIV_ERR_TOO_LARGE = 4     /* mpdiv_batch_noalloc: batch above MPDIV_NOALLOC_MAX_BATCH */
 };
@@ -67,6 +72,12 @@ enum {
  * warp per division, and passes its iterate (batch x 272 limbs) through a stream-ordered allocation from a
  * library-owned memory pool of the current device (created on first use, never destroyed; freed rows stay
  * in the pool).  Everything is enqueued on `stream`; nothing synchronises.
+ * Rows travel between HBM and shared memory as 1-D bulk asynchronous copies (cp.async.bulk + mbarrier).
+ * MPDIV_MAX_OPERAND_LIMBS < u_limbs <= MPDIV_MAX_LIMBS (2^19 bits; v_limbs <= MPDIV_MAX_OPERAND_LIMBS): the dividend
+ * stays in HBM.  The quotient is produced t = 2048 limbs at a time (1024 or 512 if shared memory is short) from a
+ * window x = r' B^t + (next t limbs of u), r' the running remainder: x < v B^t, so one shifted inverse
+ * Shinv(v, k + 1 + t) of t + 2 limbs serves every window, and each window is the division above on a
+ * (k + 1 + t)-limb dividend.  An instance whose quotient has at most t limbs is a single window.  Exact like the rest.
  */
 int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                 uint32_t *q, uint32_t *r, int batch, mpdiv_stream_t stream);
@@ -106,7 +117,7 @@ int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v
  *   MPDIV_FLAG_NO_HEAD     the head of Refine stays inside the division kernel (see mpdiv_batch_launches)
  *   MPDIV_FLAG_NO_MMA      every product of the division runs on the IMAD engine (no tcgen05 range products)
  *   MPDIV_FLAG_NO_CLUSTER  a small batch keeps one block per division (no thread-block cluster per division)
- *   MPDIV_FLAG_THREADS(n)  block size override, n in {64, 128, 256, 512}
+ *   MPDIV_FLAG_THREADS(n)  block size override, n in {32, 64, 128, 256, 512}
  */
 #define MPDIV_VARIANT_PRINTED 0
 #define MPDIV_VARIANT_CLIPPED 1
@@ -116,7 +127,7 @@ int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v
 #define MPDIV_FLAG_NO_HEAD 0x20
 #define MPDIV_FLAG_NO_MMA 0x40
 #define MPDIV_FLAG_NO_CLUSTER 0x80
-#define MPDIV_FLAG_THREADS(n) ((n) == 64 ? 0x100 : (n) == 128 ? 0x200 : (n) == 256 ? 0x300 : (n) == 512 ? 0x400 : 0)
+#define MPDIV_FLAG_THREADS(n) ((n) == 64 ? 0x100 : (n) == 128 ? 0x200 : (n) == 256 ? 0x300 : (n) == 512 ? 0x400 : (n) == 32 ? 0x500 : 0)
 #define MPDIV_FLAG_THREADS_MASK 0x700
 int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                    uint32_t *q, uint32_t *r, int batch, int flags, mpdiv_stream_t stream);
@@ -153,7 +164,7 @@ int mpmul_batch_ex(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limb
  * i.e. the UNCORRECTED Newton result of the algorithm as printed (MPDIV_VARIANT_PRINTED), so that its time
  * is the "2..4 multiplications" of the cost model.
  *   v : batch x v_limbs (device, read);  w : batch x w_limbs (device, written),
- * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_LIMBS.  v_i = 0 gives w_i = all ones (status bit MPDIV_STATUS_V_ZERO).
+ * w_limbs >= h + 1, 1 <= h <= MPDIV_MAX_OPERAND_LIMBS.  v_i = 0 gives w_i = all ones (status bit MPDIV_STATUS_V_ZERO).
  */
 int shinv_batch(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_limbs,
                 int batch, mpdiv_stream_t stream);
@@ -239,11 +250,13 @@ int mpdiv_mma_probe(int n_cols, int issuers, int iters, int form, unsigned long 
  *   MPDIV_STATUS_REM_RANGE   clipped variant: the remainder estimate u - v*q0' left the range the
  *                            mod-B^(k+3) arithmetic assumes (its top limb is neither 0 nor all ones): NOT exact
  *   MPDIV_STATUS_V_ZERO      a divisor was zero (undefined): q = all ones, r = low limbs of u
+ *   MPDIV_STATUS_IO_WAIT     a bounded wait for a bulk copy of an operand row gave up: NOT exact
  */
 #define MPDIV_STATUS_MMA_WAIT 1u
 #define MPDIV_STATUS_CORR_BOUND 2u
 #define MPDIV_STATUS_REM_RANGE 4u
 #define MPDIV_STATUS_V_ZERO 8u
+#define MPDIV_STATUS_IO_WAIT 16u
 int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset);
 
 /*
@@ -265,7 +278,8 @@ int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset);
  *          Refine from the 17-digit seed (mpdiv_seed_batch)
  *   out[16] tensor-core work: sum over range products of (MMA steps x accumulator columns); x 16384 = the
  *          u8 x u8 multiply-accumulates the tensor pipe executed (4 instructions of M = 128, K = 32 per step)
- *   out[17] divisions that ran on a thread-block cluster      out[18..23] reserved (0)
+ *   out[17] reserved (0)      out[18] quotient windows of the chunked form (dividends above MPDIV_MAX_OPERAND_LIMBS
+ *          limbs)      out[19..23] reserved (0)
  */
 #define MPDIV_NUM_COUNTERS 24
 int mpdiv_debug_counters(unsigned long long out[MPDIV_NUM_COUNTERS], int reset, mpdiv_stream_t stream);

@@ -23,17 +23,18 @@ VARIANT_PRINTED, VARIANT_CLIPPED = 0, 1
 VARIANT_DEFAULT = VARIANT_CLIPPED
 # tuning switches OR-ed into the `flags` of the *_ex calls (include/mpdiv.h)
 FLAG_NO_SEED, FLAG_NO_HEAD, FLAG_NO_MMA, FLAG_NO_CLUSTER = 0x10, 0x20, 0x40, 0x80
-STATUS_MMA_WAIT, STATUS_CORR_BOUND, STATUS_REM_RANGE, STATUS_V_ZERO = 1, 2, 4, 8
+STATUS_MMA_WAIT, STATUS_CORR_BOUND, STATUS_REM_RANGE, STATUS_V_ZERO, STATUS_IO_WAIT = 1, 2, 4, 8, 16
 NUM_COUNTERS = 24
 
 
 def flag_threads(n: int) -> int:
     """MPDIV_FLAG_THREADS(n): block size override."""
-    return {64: 0x100, 128: 0x200, 256: 0x300, 512: 0x400}[int(n)]
+    return {32: 0x500, 64: 0x100, 128: 0x200, 256: 0x300, 512: 0x400}[int(n)]
 
 ENGINE_IMAD, ENGINE_TENSOR = 0, 1
 LINOP_ADD, LINOP_SUB, LINOP_NEG, LINOP_SHIFT, LINOP_PREC, LINOP_ANY = range(6)
-MAX_LIMBS = 8192
+MAX_LIMBS = 16384          # u_limbs of mpdiv_batch (default variant)
+MAX_OPERAND_LIMBS = 8192   # every other stride
 
 
 class MpdivError(RuntimeError):
@@ -283,7 +284,7 @@ def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, form: int = 0, s
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
                  "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "mma_products", "mma_wait_failures",
-                 "seed_addbacks", "seeds", "mma_colsteps", "cluster_divs")
+                 "seed_addbacks", "seeds", "mma_colsteps", "cluster_divs", "chunks")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:

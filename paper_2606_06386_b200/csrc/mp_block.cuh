@@ -25,7 +25,7 @@ constexpr int CHUNK = 8;       // limbs per thread in linear operations
 __host__ __device__ constexpr int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // Sticky status word (include/mpdiv.h: mpdiv_status): conditions only a running kernel can find.
-enum : uint32_t { ST_MMA_WAIT = 1u, ST_CORR_BOUND = 2u, ST_REM_RANGE = 4u, ST_V_ZERO = 8u };
+enum : uint32_t { ST_MMA_WAIT = 1u, ST_CORR_BOUND = 2u, ST_REM_RANGE = 4u, ST_V_ZERO = 8u, ST_IO_WAIT = 16u };
 __device__ unsigned int g_status;
 __device__ __forceinline__ void raise_status(uint32_t bits)
 {
@@ -38,7 +38,7 @@ __device__ unsigned long long g_counters[NUM_COUNTERS];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
        CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
        CNT_MMA_PRODUCTS, CNT_MMA_WAIT_FAILURES /* filled by the host from mp_mma.cuh */, CNT_SEED_ADDBACK, CNT_SEEDS,
-       CNT_MMA_COLSTEPS, CNT_CLUSTER_DIVS };
+       CNT_MMA_COLSTEPS, CNT_CLUSTER_DIVS, CNT_CHUNKS };
 __device__ __forceinline__ void count(int which, unsigned long long n = 1ull)
 {
     if (threadIdx.x == 0) atomicAdd(&g_counters[which], n);
@@ -47,6 +47,8 @@ __device__ __forceinline__ void count(int which, unsigned long long n = 1ull)
 // Per-block bookkeeping for the scans/reductions: a double-buffered word per warp.
 struct BlkScratch {
     uint32_t code[2][32];
+    unsigned long long io_bar;   // mbarrier of the block's bulk copies (mp_io.cuh)
+    uint32_t pad_[2];            // keeps whatever follows 16-byte aligned
 };
 
 struct Blk {

@@ -11,39 +11,11 @@
 #include "mp_block.cuh"
 #include "mp_mul.cuh"
 #include "mp_div.cuh"
+#include "mp_io.cuh"
 
 using namespace mpd;
 
 #define MPDIV_VERSION_STR "mpdiv 0.6 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
-
-// ---------------------------------------------------------------------------------------
-// global <-> shared staging
-// ---------------------------------------------------------------------------------------
-// dst[0..n) = src[0..n) with 128-bit coalesced loads (n multiple of 4), dst[n..pad) = 0.
-template <int T>
-__device__ __forceinline__ void load_number(limb *dst, const limb *__restrict__ src, int n, int pad)
-{
-    const uint4 *s4 = reinterpret_cast<const uint4 *>(src);
-    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
-    for (int i = threadIdx.x; i < n / 4; i += T) d4[i] = __ldg(s4 + i);
-    for (int i = n + (int)threadIdx.x; i < pad; i += T) dst[i] = 0u;
-}
-
-// dst[0..n) = (i < valid) ? src[i] : 0, 128-bit coalesced stores; valid multiple of 4 not required.
-template <int T>
-__device__ __forceinline__ void store_number(limb *__restrict__ dst, const limb *src, int n, int valid)
-{
-    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
-    for (int i = threadIdx.x; i < n / 4; i += T) {
-        const int b = 4 * i;
-        uint4 x;
-        x.x = (b + 0 < valid) ? src[b + 0] : 0u;
-        x.y = (b + 1 < valid) ? src[b + 1] : 0u;
-        x.z = (b + 2 < valid) ? src[b + 2] : 0u;
-        x.w = (b + 3 < valid) ? src[b + 3] : 0u;
-        d4[i] = x;
-    }
-}
 
 // ---------------------------------------------------------------------------------------
 // mpmul_batch
@@ -263,7 +235,7 @@ Tune tune_of(int flags)
     t.no_mma = (flags & MPDIV_FLAG_NO_MMA) != 0;
     t.no_cluster = (flags & MPDIV_FLAG_NO_CLUSTER) != 0;
     const int c = (flags & MPDIV_FLAG_THREADS_MASK) >> 8;
-    t.threads = c >= 1 && c <= 4 ? 32 << c : 0;
+    t.threads = c >= 1 && c <= 4 ? 32 << c : (c == 5 ? 32 : 0);
     t.wmid_fixed = nullptr;
     return t;
 }
@@ -273,16 +245,23 @@ bool flags_ok(int flags)
     if (var != MPDIV_VARIANT_PRINTED && var != MPDIV_VARIANT_CLIPPED) return false;
     if (flags & ~(MPDIV_VARIANT_MASK | MPDIV_FLAG_NO_SEED | MPDIV_FLAG_NO_HEAD | MPDIV_FLAG_NO_MMA | MPDIV_FLAG_NO_CLUSTER |
                   MPDIV_FLAG_THREADS_MASK)) return false;
-    return ((flags & MPDIV_FLAG_THREADS_MASK) >> 8) <= 4;
+    return ((flags & MPDIV_FLAG_THREADS_MASK) >> 8) <= 5;
 }
 
 // threads per block for numbers of `limbs` limbs.  Four lanes share a tile diagonal (mp_mul.cuh), so
 // a block of T threads covers T/4 diagonals = 2T limbs of product per pass.  256 threads at 128
 // registers let two blocks share an SM up to 4096 limbs; above that one block of 512 fills the SM.
-int threads_for(int limbs, int override_threads = 0)
+// sched = the divisions that share the GPU (0 = unknown).  Small numbers in large batches (the
+// paper's "suboptimal number of threads per CUDA block" below 2^15 bits): a block is too big
+// a unit, so a division gets ONE WARP (32-thread blocks, 16 resident per SM, warp-level barriers only) up to 512
+// limbs and two warps at 1024 -- measured on 4736-9472 divisions: 68.6 M div/s against 40.4 M at 32 limbs, 27.3 M
+// against 12.3 M at 256, 16.3 M against 11.4 M at 512, 7.84 M against 7.15 M at 1024 limbs.
+int threads_for(int limbs, int override_threads = 0, int sched = 0)
 {
     if (override_threads) return override_threads;
+    if (limbs <= 512 && sched >= 16 * g_sm_count) return 32;
     if (limbs <= 128) return 64;
+    if (limbs <= 1024 && sched >= 8 * g_sm_count) return 64;
     if (limbs <= 2048) return 128;      // four blocks per SM overlap the latency-bound early iterations
     if (limbs <= 4096) return 256;
     return 512;
@@ -339,7 +318,7 @@ int mpmul_batch_ex(const uint32_t *a, int a_limbs, const uint32_t *b, int b_limb
     if ((a_limbs | b_limbs | c_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (!aligned16(a) || !aligned16(b) || !aligned16(c)) return MPDIV_ERR_BAD_ARG;
     if (c_limbs > a_limbs + b_limbs) return MPDIV_ERR_BAD_ARG;
-    if (a_limbs > MPDIV_MAX_LIMBS || b_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (a_limbs > MPDIV_MAX_OPERAND_LIMBS || b_limbs > MPDIV_MAX_OPERAND_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     if (engine == MPMUL_ENGINE_TENSOR) return launch_mul<512>(a, a_limbs, b, b_limbs, c, c_limbs, batch, st, true);

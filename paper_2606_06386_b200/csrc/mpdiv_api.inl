@@ -15,6 +15,7 @@ struct DivLayout {
     int p_words_r;    // Refine: capacity of P and of HI
     int p_words_q;    // quotient phase: capacity of P and of HI
     int hcap;         // the layout holds instances with H = max(h - k, 2) <= hcap
+    int qb_off;       // chunked form (mpdiv_kernel<.., BIG>): the quotient chunk's own buffer; otherwise = wa_off
 };
 
 // M: limbs of the dividend side (u stride, or h for shinv_batch); n: divisor stride;
@@ -55,6 +56,7 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip, int hca
     L.mma_rows = 0;
     L.mma_cols = 0;
     L.hcap = hc;
+    L.qb_off = L.wa_off;
     return L;
 }
 
@@ -109,6 +111,39 @@ static size_t div_layouts_with_mma(DivLayout &Lf, DivLayout &Lc, int u_limbs, in
     }
     Lc.total_words = Lf.total_words = end;
     return (size_t)end * 4;
+}
+
+// Layout of the CHUNKED division (mpdiv_kernel<.., BIG>; dividends above MPDIV_MAX_OPERAND_LIMBS limbs, whose rows do not
+// fit beside the divisor and the product scratch): the dividend is not resident.  The quotient is produced t limbs at a
+// time from a WINDOW of at most k + 1 + t limbs (the running remainder above the next t limbs of u, streamed from HBM),
+// with one shifted inverse of t + 2 limbs for all windows.  V | window (the U area; Refine's second iterate buffer) |
+// WA (iterates, shinv) | QB (quotient chunk) | product scratch | tensor-core scratch | mbarriers.  Sized like a regular
+// division of a (v_limbs + 1 + t)-limb dividend whose inverse has at most t + 2 limbs.  Returns the bytes, 0 when t does
+// not fit max_smem.
+static size_t div_layout_big(DivLayout &L, int v_limbs, int t, int threads, int max_smem)
+{
+    const int np = round_up(v_limbs, TILE);
+    L = div_layout(np + 1 + t + 1, v_limbs, true, true, t + 40);
+    L.qb_off = L.total_words;
+    L.total_words += round_up(t + 32, TILE);
+    const int bar_words = MMA_BAR_BYTES / 4;
+    // tensor-core scratch: v * q_chunk needs ceil((k + 3) / 32) output blocks (one accumulator set when that exceeds 256
+    // columns) and one row per block and per 128-byte chunk of the quotient chunk
+    const int blocks = (np + 8 + 31) / 32 + 1;
+    const int nn = (blocks + 15) & ~15;
+    const int want = nn > 256 ? nn : 2 * nn;
+    const int cols = want <= 32 ? 32 : want <= 64 ? 64 : want <= 128 ? 128 : want <= 256 ? 256 : 512;
+    const int rows = round_up(nn + (t + 2 + 31) / 32 + 2, 8);
+    const int off = round_up(L.total_words, 256);
+    const int end = off + mma_scratch_bytes(rows, threads) / 4;
+    if (nn <= 512 && (end + bar_words) * 4 <= max_smem) {
+        L.mma_off = off;
+        L.mma_rows = rows;
+        L.mma_cols = cols;
+        L.bar_off = end;
+        L.total_words = end + bar_words;
+    }
+    return (size_t)L.total_words * 4 <= (size_t)max_smem ? (size_t)L.total_words * 4 : 0;
 }
 
 __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout &L)
@@ -247,23 +282,59 @@ constexpr int CORR_MAX = 64;
 template <int T, bool LAT>
 struct DivMma { static constexpr bool value = MmaEnabled<T>::value && !(LAT && T <= 128); };
 
+// significant limbs of a row in global memory (n a multiple of 4, 16-byte aligned), by the whole block
+template <int T>
+__device__ __forceinline__ int global_prec(const limb *__restrict__ a, int n, Blk &blk)
+{
+    const uint4 *a4 = reinterpret_cast<const uint4 *>(a);
+    int top = 0;
+    for (int i = threadIdx.x; i < n / 4; i += T) {
+        const uint4 x = __ldg(a4 + i);
+        if (x.x | x.y | x.z | x.w) top = 4 * i + (x.w ? 4 : x.z ? 3 : x.y ? 2 : 1);
+    }
+    return block_max<T>(top, blk);
+}
+
+// dst[0..n) = (i < valid) ? src[i] : 0, both rows in global memory (n a multiple of 4, 16-byte aligned)
+template <int T>
+__device__ __forceinline__ void copy_row_global(limb *__restrict__ dst, const limb *__restrict__ src, int n, int valid)
+{
+    const uint4 *s4 = reinterpret_cast<const uint4 *>(src);
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+    for (int i = threadIdx.x; i < n / 4; i += T) {
+        const int b = 4 * i;
+        uint4 x = (b < valid) ? __ldg(s4 + i) : make_uint4(0u, 0u, 0u, 0u);
+        if (b + 1 >= valid) x.y = 0u;
+        if (b + 2 >= valid) x.z = 0u;
+        if (b + 3 >= valid) x.w = 0u;
+        d4[i] = x;
+    }
+}
+
 // MMA = this instantiation carries the engine (at most DivMma<T, LAT>; 128-thread throughput blocks also exist
 // without it, for the sizes that never use it: its mere presence costs 2^15-bit batches 4 %).
-template <int T, bool LAT, bool MMA>
+// BIG = the chunked form for dividends that do not fit on chip (div_layout_big: the
+// paper stops at 2^18 bits for lack of shared memory).  u stays in HBM; with D = h - k quotient limbs to produce and
+// chunks of t limbs, chunk c (from the top) divides the window x_c = r_(c-1) B^t + (the next t limbs of u) by v:
+// x_c < v B^t, so its quotient has t limbs, and ONE inverse w = Shinv(v, k + 1 + t) serves every window
+// (q0 = floor(x w / B^(k+1+t)) is within the range of the bounded correction loops for any x < B^(k+1+t)).
+// A division with D <= t is a single window with h_w = h: exactly the resident algorithm.
+template <int T, bool LAT, bool MMA, bool BIG = false>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, DivLayout Lc, int clip, int narrow_l,
-             const limb *__restrict__ wmid)
+             const limb *__restrict__ wmid, int tchunk)
 {
     // L: the layout for any instance of these strides; Lc: the compact layout (H <= Lc.hcap); each with the tensor-core
-    // scratch behind it or mma_off < 0 (div_layouts_with_mma).  V, U and the block scratch coincide.
+    // scratch behind it or mma_off < 0 (div_layouts_with_mma).  V, U and the block scratch coincide.  BIG: L == Lc.
     extern __shared__ __align__(1024) uint32_t smem[];
     limb *V = smem + L.v_off;          // divisor at V + 4 (one-limb divisors are re-based to V)
-    limb *U = smem + L.u_off;          // dividend at U + 4 (same)
+    limb *U = smem + L.u_off;          // dividend (BIG: the window) at U + 4 (same)
     limb *WA = smem + L.wa_off;        // shinv, then the quotient
     Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
     static_assert(!MMA || DivMma<T, LAT>::value, "no tensor-core engine for this block size");
+    static_assert(!BIG || !LAT, "the chunked form is a throughput kernel");
     MmaCtx mcx;
     MmaCtx *mma = nullptr;
     if constexpr (MMA) {
@@ -275,32 +346,41 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             mma_decline();
         }
     }
+    IoBar io;
+    io_init<T>(io, blk.sc);
 
     for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
         const limb *ug = u + (size_t)inst * u_limbs;
+        const limb *vg = v + (size_t)inst * v_limbs;
         limb *qg = q + (size_t)inst * u_limbs;
         limb *rg = r + (size_t)inst * v_limbs;
 
-        // a1/a2: load, precisions ("h <- prec(u)")
-        load_number<T>(V + 4, v + (size_t)inst * v_limbs, v_limbs, vpad - 4);
-        load_number<T>(U + 4, ug, u_limbs, upad - 4);
+        // a1/a2: load (one bulk copy per row), precisions ("h <- prec(u)")
         if (threadIdx.x < 4) { V[threadIdx.x] = 0u; U[threadIdx.x] = 0u; }
-        __syncthreads();
+        int h;
+        if constexpr (BIG) {
+            load_rows<T>(io, V + 4, vg, v_limbs, vpad - 4, nullptr, nullptr, 0, 0);
+            h = global_prec<T>(ug, u_limbs, blk);
+        } else {
+            load_rows<T>(io, V + 4, vg, v_limbs, vpad - 4, U + 4, ug, u_limbs, upad - 4);
+            h = prec_of<T>(U + 4, u_limbs, blk);
+        }
         const int pv = prec_of<T>(V + 4, v_limbs, blk);
-        int h = prec_of<T>(U + 4, u_limbs, blk);
 
         if (pv == 0) {                                     // v = 0: q = all ones, r = low limbs of u
             count(CNT_V_ZERO);
             raise_status(ST_V_ZERO);
             for (int i = threadIdx.x; i < u_limbs; i += T) qg[i] = 0xffffffffu;
-            store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
+            if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, min(u_limbs, v_limbs));
+            else store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
             __syncthreads();
             continue;
         }
         if (pv > h) {                                      // u < v: (0, u)
             count(CNT_U_LT_V);
-            store_number<T>(qg, U + 4, u_limbs, 0);
-            store_number<T>(rg, U + 4, v_limbs, h);
+            store_row<T>(qg, U + 4, u_limbs, 0);
+            if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, h);
+            else store_number<T>(rg, U + 4, v_limbs, h);
             __syncthreads();
             continue;
         }
@@ -319,7 +399,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
 
         // the layout of this instance: compact (and with it the tensor-core engine) when its inverse and quotient are
         // short enough, the full one otherwise
-        const bool compact = mma != nullptr && max(h - k, 2) <= Lc.hcap;
+        const bool compact = BIG || (mma != nullptr && max(h - k, 2) <= Lc.hcap);
         const DivLayout &Li = compact ? Lc : L;
         MmaCtx *mma_i = (mma != nullptr && Li.mma_off >= 0) ? mma : nullptr;
         if (mma_i) {                                       // the scratch of this instance's layout
@@ -334,25 +414,55 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         mq.OV = mq.HI + Li.p_words_q;
         mq.C3 = mq.OV + round_up(Li.p_words_q / TILE, 4);
 
+        // chunks of the quotient (BIG; otherwise one window = the whole dividend)
+        const int D = h - k;                               // q < B^D
+        const int nchunks = BIG ? max(1, (D + tchunk - 1) / tchunk) : 1;
+        const int hx = (BIG && nchunks > 1) ? k + 1 + tchunk : h;     // every window is < B^hx
+
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
-        const int nw = shinv_block<T, MMA>(Vb, k, h, rb, blk, clip != 0, mma_i, narrow_l & 255, !(narrow_l & 256),
+        const int nw = shinv_block<T, MMA>(Vb, k, hx, rb, blk, clip != 0, mma_i, narrow_l & 255, !(narrow_l & 256),
                                       (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
 
-        // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
-        if (one_limb) {
-            for (int i = threadIdx.x; i < upad; i += T)
-                U[i] = (i >= 1 && i <= u_limbs) ? __ldg(ug + i - 1) : 0u;
-            Ub = U;
-        } else {
-            load_number<T>(U + 4, ug, u_limbs, upad - 4);
-        }
-        __syncthreads();
-        const int nq = h - k + 1;                          // q0 <= B^(h-k): at most h-k+1 limbs
+        const int nq = hx - k + 1;                         // q0 <= B^(hx-k): at most hx-k+1 limbs
         const int qlen = round_up(nq + 1, TILE);
-        limb *Q = WA;
+        limb *Q = BIG ? smem + Li.qb_off : WA;             // resident form: WA (shinv) is dead once q0 is formed
         limb *R = PQ, *R2 = mq.HI;                         // r in place over p; HI is free after the product
-        int rlen;                                          // limbs of the remainder arithmetic
+        int rlen = 0;                                      // limbs of the remainder arithmetic
+
+        for (int c = 0; c < nchunks; ++c) {
+        const int lo = BIG ? (nchunks - 1 - c) * tchunk : 0;          // this chunk gives the quotient limbs from lo up
+        if constexpr (BIG) {
+            // the window: x_c = r_(c-1) B^t + u[lo, lo + t), or the top h - lo limbs of u for c = 0
+            const int nu = (c == 0) ? h - lo : tchunk;                // limbs taken from u (h counts the B of u*B)
+            const int wtop = round_up(hx + 1, TILE) + 8;
+            const int n4 = one_limb ? nu : min(round_up(nu, 4), u_limbs - lo);   // limbs of u above h are zero
+            if (c > 0) {
+                for (int i = threadIdx.x; i < wtop - tchunk; i += T) Ub[tchunk + i] = (i <= k) ? R[i] : 0u;
+            } else {
+                for (int i = n4 + (int)threadIdx.x; i < wtop; i += T) Ub[i] = 0u;
+            }
+            if (one_limb) {                                // limb i of u*B is limb i - 1 of u
+                for (int i = threadIdx.x; i < nu; i += T) {
+                    const int j = lo + i - 1;
+                    Ub[i] = (j >= 0 && j < u_limbs) ? __ldg(ug + j) : 0u;
+                }
+                __syncthreads();
+            } else {
+                load_rows<T>(io, Ub, ug + lo, n4, n4, nullptr, nullptr, 0, 0);
+            }
+            R = PQ; R2 = mq.HI;
+        } else {
+            // reload u; for one-limb divisors u*B, re-based to the aligned U (limb i of u at U[i+1])
+            if (one_limb) {
+                for (int i = threadIdx.x; i < upad; i += T)
+                    U[i] = (i >= 1 && i <= u_limbs) ? __ldg(ug + i - 1) : 0u;
+                Ub = U;
+                __syncthreads();
+            } else {
+                load_rows<T>(io, U + 4, ug, u_limbs, upad - 4, nullptr, nullptr, 0, 0);
+            }
+        }
         int minus = 0;
         if (!clip) {
             // a9: q0 = shift_{-h}(u * shinv)  (Alg. 3 line 2); the full product, as printed
@@ -382,24 +492,24 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                 lin_addsub<T, true>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
             }
         } else {
-            // a9 clipped: only the columns >= h - 9 of u * shinv; q0' in {q0 - 1, q0}
+            // a9 clipped: only the columns >= hx - 9 of x * shinv; q0' in {q0 - 1, q0}
             if (psh == 0) {
                 lin_zero<T>(Q, qlen);
             } else {
-                const int dlo = (h - 1) / 32;              // tensor-core form: E < B^(32 dlo + 1) <= B^h
-                int pl = try_mma_range<T, MMA>(mma_i, Ub, h, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
+                const int dlo = (hx - 1) / 32;             // tensor-core form: E < B^(32 dlo + 1) <= B^hx
+                int pl = try_mma_range<T, MMA>(mma_i, Ub, hx, WA, psh, dlo, 1 << 20, PQ, mq.HI, blk);
                 if (pl >= 0) {
                     count(CNT_MMA_PRODUCTS);
-                    lin_copy<T>(Q, qlen, PQ, pl, h - 32 * dlo);
+                    lin_copy<T>(Q, qlen, PQ, pl, hx - 32 * dlo);
                 } else {
-                    const int Klo = (h >= 17) ? (h - 9) / TILE : 0;
-                    pl = mul_range<T>(Ub, h, WA, psh, Klo, 1 << 20, PQ, mq, blk);
-                    lin_copy<T>(Q, qlen, PQ, pl, h - TILE * Klo);
+                    const int Klo = (hx >= 17) ? (hx - 9) / TILE : 0;
+                    pl = mul_range<T>(Ub, hx, WA, psh, Klo, 1 << 20, PQ, mq, blk);
+                    lin_copy<T>(Q, qlen, PQ, pl, hx - TILE * Klo);
                 }
             }
             const int pq = top_prec(Q, nq);
 
-            // a10 clipped: |u - v q0'| < 4v < B^(k+2), so the remainder arithmetic runs mod B^rlen
+            // a10 clipped: |x - v q0'| < 4v < B^(k+2), so the remainder arithmetic runs mod B^rlen
             rlen = round_up(k + 3, TILE);
             int pl = 0;
             if (pq > 0) {
@@ -412,8 +522,8 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                     pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
                 }
             }
-            // a11: r = u - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
-            lin_addsub<T, true>(R, rlen, LimbView{Ub, h, 0}, LimbView{PQ, pl, 0}, 0u, blk);
+            // a11: r = x - p (mod B^rlen); negative (top limb all ones) -> q - 1, r + v
+            lin_addsub<T, true>(R, rlen, LimbView{Ub, hx, 0}, LimbView{PQ, pl, 0}, 0u, blk);
             // the estimate must lie in (-B^(k+2), B^(k+2)): its top limb (index >= k+2) is 0 or all ones
             if (R[rlen - 1] != 0u && R[rlen - 1] != 0xffffffffu) raise_status(ST_REM_RANGE);
             while (R[rlen - 1] != 0u && minus < CORR_MAX) {
@@ -440,10 +550,24 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             raise_status(ST_CORR_BOUND);
         }
 
-        // a12: store (remainder of the scaled problem is r*B for one-limb divisors)
-        store_number<T>(qg, Q, u_limbs, min(qlen, u_limbs));
+        // a12: the quotient limbs of this window (everything above the top window is zero)
+        if constexpr (BIG) {
+            if (c == 0) {
+                store_row<T>(qg + lo, Q, u_limbs - lo, min(qlen, u_limbs - lo));
+            } else {
+                if (Q[tchunk] != 0u) raise_status(ST_CORR_BOUND);     // x_c < v B^t: the quotient has t limbs
+                store_row<T>(qg + lo, Q, tchunk, tchunk);
+            }
+            count(CNT_CHUNKS);
+            __syncthreads();
+        } else {
+            store_row<T>(qg, Q, u_limbs, min(qlen, u_limbs));
+        }
+        }   // chunks
+
+        // a12: the remainder (of the scaled problem it is r*B for one-limb divisors)
         if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
-        else store_number<T>(rg, R, v_limbs, min(k + 1, v_limbs));
+        else store_row<T>(rg, R, v_limbs, min(round_up(k + 1, 4), v_limbs));
         __syncthreads();
     }
     count_tiles(blk);
@@ -564,10 +688,32 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
             shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
         }
     }
-    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid);
+    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid, 0);
     const bool ok = cudaGetLastError() == cudaSuccess;
     if (wmid && !tn.wmid_fixed) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
+}
+
+// Dividends above MPDIV_MAX_OPERAND_LIMBS limbs: the chunked form (mpdiv_kernel<512, false, true, true>), clipped variant
+// only, divisor strides up to MPDIV_MAX_OPERAND_LIMBS.  The chunk is the largest of 2048, 1024, 512 limbs whose layout fits.
+int launch_div_big(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+                   cudaStream_t st, int sched, const Tune &tn)
+{
+    constexpr int T = 512;
+    DivLayout L;
+    size_t bytes = 0;
+    int t = 2048;
+    for (; t >= 512; t /= 2) {
+        bytes = div_layout_big(L, v_limbs, t, T, g_max_smem);
+        if (bytes) break;
+    }
+    if (!bytes) return MPDIV_ERR_UNSUPPORTED;
+    if (tn.no_mma) L.mma_off = -1;
+    int rc = set_smem(mpdiv_kernel<T, false, true, true>, bytes);
+    if (rc != MPDIV_OK) return rc;
+    mpdiv_kernel<T, false, true, true><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, L, 1, narrow_for(sched, tn),
+                                                                nullptr, t);
+    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
 template <int T, bool LAT>
@@ -592,8 +738,10 @@ int launch_div(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, 
 {
     // a batch that fits the SMs at the latency kernel's occupancy (two blocks per SM up to 128 threads, one at
     // 256) is latency bound: give its threads all the registers they want
-    if (T <= 256 && sched <= (T <= 128 ? 2 : 1) * g_sm_count)
-        return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+    if constexpr (T <= 256) {
+        if (sched <= (T <= 128 ? 2 : 1) * g_sm_count)
+            return launch_div_k<T, true>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
+    }
     return launch_div_k<T, false>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
 }
 
@@ -614,7 +762,7 @@ int check_div_args(const void *u, int u_limbs, const void *v, int v_limbs, const
 {
     if (!u || !v || !q || !r || u_limbs <= 0 || v_limbs <= 0 || batch <= 0) return MPDIV_ERR_BAD_ARG;
     if ((u_limbs | v_limbs) & 3) return MPDIV_ERR_BAD_ARG;
-    if (u_limbs > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (u_limbs > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_OPERAND_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     return MPDIV_OK;
 }
 
@@ -631,7 +779,12 @@ int mpdiv_batch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, 
 static int div_dispatch(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs, uint32_t *q, uint32_t *r,
                         int batch, int clip, cudaStream_t st, int sched, const Tune &tn)
 {
-    switch (threads_for(u_limbs, tn.threads)) {
+    if (u_limbs > MPDIV_MAX_OPERAND_LIMBS) {                   // the dividend does not fit on chip: chunked form
+        if (!clip) return MPDIV_ERR_UNSUPPORTED;
+        return launch_div_big(u, u_limbs, v, v_limbs, q, r, batch, st, sched, tn);
+    }
+    switch (threads_for(u_limbs, tn.threads, sched)) {
+        case 32: return launch_div<32>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
         case 64: return launch_div<64>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
         case 128: return launch_div<128>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
         case 256: return launch_div<256>(u, u_limbs, v, v_limbs, q, r, batch, st, clip, sched, tn);
@@ -668,7 +821,7 @@ int shinv_batch_ex(const uint32_t *v, int v_limbs, int h, uint32_t *w, int w_lim
     if ((v_limbs | w_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (w_limbs < h + 1) return MPDIV_ERR_BAD_ARG;
     if (!aligned16(v) || !aligned16(w)) return MPDIV_ERR_BAD_ARG;
-    if (h > MPDIV_MAX_LIMBS || v_limbs > MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (h > MPDIV_MAX_OPERAND_LIMBS || v_limbs > MPDIV_MAX_OPERAND_LIMBS) return MPDIV_ERR_UNSUPPORTED;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     switch (threads_for(h, tn.threads)) {
@@ -687,8 +840,8 @@ int mplinop_batch(int op, const uint32_t *a, int a_limbs, const uint32_t *b, int
     if (op < MPLINOP_ADD || op > MPLINOP_ANY) return MPDIV_ERR_BAD_ARG;
     if ((a_limbs | b_limbs | out_limbs) & 3) return MPDIV_ERR_BAD_ARG;
     if (!aligned16(a) || !aligned16(b) || !aligned16(out)) return MPDIV_ERR_BAD_ARG;
-    if (a_limbs > MPDIV_MAX_LIMBS || b_limbs > MPDIV_MAX_LIMBS || out_limbs > 2 * MPDIV_MAX_LIMBS) return MPDIV_ERR_UNSUPPORTED;
-    if (shift < -2 * MPDIV_MAX_LIMBS || shift > 2 * MPDIV_MAX_LIMBS) return MPDIV_ERR_BAD_ARG;
+    if (a_limbs > MPDIV_MAX_OPERAND_LIMBS || b_limbs > MPDIV_MAX_OPERAND_LIMBS || out_limbs > 2 * MPDIV_MAX_OPERAND_LIMBS) return MPDIV_ERR_UNSUPPORTED;
+    if (shift < -2 * MPDIV_MAX_OPERAND_LIMBS || shift > 2 * MPDIV_MAX_OPERAND_LIMBS) return MPDIV_ERR_BAD_ARG;
     if ((op == MPLINOP_NEG && (shift < 0 || shift > out_limbs)) || (op == MPLINOP_ANY && shift < 0)) return MPDIV_ERR_BAD_ARG;
     if (!device_props()) return MPDIV_ERR_CUDA;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -816,7 +969,8 @@ int mpdiv_batch_launches(int u_limbs, int batch, int flags)
 {
     if (u_limbs <= 0 || batch <= 0 || !flags_ok(flags) || !device_props()) return 0;
     const Tune tn = tune_of(flags);
-    const int T = threads_for(u_limbs, tn.threads);
+    if (u_limbs > MPDIV_MAX_OPERAND_LIMBS) return 1;
+    const int T = threads_for(u_limbs, tn.threads, batch);
     const bool lat = T <= 256 && batch <= (T <= 128 ? 2 : 1) * g_sm_count;
     return use_head(u_limbs, (flags & MPDIV_VARIANT_MASK) == MPDIV_VARIANT_CLIPPED, lat, tn) ? 2 : 1;
 }
@@ -851,7 +1005,8 @@ int mpdiv_debug_counters(unsigned long long out[MPDIV_NUM_COUNTERS], int reset, 
 int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset)
 {
     static_assert(MPDIV_STATUS_MMA_WAIT == ST_MMA_WAIT && MPDIV_STATUS_CORR_BOUND == ST_CORR_BOUND &&
-                  MPDIV_STATUS_REM_RANGE == ST_REM_RANGE && MPDIV_STATUS_V_ZERO == ST_V_ZERO, "status bits agree");
+                  MPDIV_STATUS_REM_RANGE == ST_REM_RANGE && MPDIV_STATUS_V_ZERO == ST_V_ZERO && MPDIV_STATUS_IO_WAIT == ST_IO_WAIT,
+                  "status bits agree");
     if (!flags) return MPDIV_ERR_BAD_ARG;
     if (cudaStreamSynchronize(reinterpret_cast<cudaStream_t>(stream)) != cudaSuccess) return MPDIV_ERR_CUDA;
     if (cudaMemcpyFromSymbol(flags, g_status, sizeof(unsigned int)) != cudaSuccess) return MPDIV_ERR_CUDA;

@@ -306,6 +306,31 @@ def test_div_random_effective_precisions_large(variant):
     check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, M), "random precisions 2048", variant)
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("M,n,threads", [(8, 4, 32), (32, 32, 32), (64, 32, 32), (128, 64, 32), (256, 128, 32), (512, 256, 32),
+                                         (1024, 512, 32), (1024, 512, 64), (512, 512, 64), (100, 52, 32)])
+def test_div_one_warp_per_division(M, n, threads, variant):
+    """small numbers in large batches get one warp (32-thread blocks) or two per division instead of a
+    128-thread block.  Forced here through MPDIV_FLAG_THREADS on the directed set; every primitive runs
+    in its warp form."""
+    u, v = inputs.directed(M, n, count=768)
+    check_div(u, v, "directed M=%d n=%d T=%d" % (M, n, threads), variant | binding.flag_threads(threads))
+
+
+@pytest.mark.parametrize("M,n,batch", [(64, 32, 4736), (256, 128, 4736), (512, 256, 2400), (1024, 512, 1200)])
+def test_div_small_numbers_large_batches_default_mapping(M, n, batch):
+    """The mapping mpdiv_batch picks by itself for batches of at least 16 (8) divisions per SM: random effective
+    precisions, default variant."""
+    rng = inputs.rng_for(402, M)
+    us, vs = [], []
+    for i in range(batch):
+        lv = int(rng.integers(1, n + 1))
+        lu = int(rng.integers(0, M + 1))
+        us.append(inputs._random_int(rng, lu))
+        vs.append(inputs._random_int(rng, lv))
+    check_div(inputs.ints_to_rows(us, M), inputs.ints_to_rows(vs, n), "random precisions %d/%d x %d" % (M, n, batch))
+
+
 def test_div_uses_tensor_engine_at_2_16_bits_in_throughput_batches_only():
     """128-thread blocks: a throughput batch of config 2's shape runs its large range products on the tensor core
     (warp 0 produces and issues, mp_mma.cuh); the latency kernel of a small batch is compiled without the engine.
@@ -399,7 +424,7 @@ def test_bad_arguments_are_rejected():
     with pytest.raises(binding.MpdivError) as e:
         binding.mpdiv_batch(du[:, :6].contiguous(), dv)           # stride not a multiple of 4
     assert e.value.code == binding.ERR_BAD_ARG
-    big = torch.zeros((1, 8196), dtype=torch.int32, device="cuda")
+    big = torch.zeros((1, 16388), dtype=torch.int32, device="cuda")
     with pytest.raises(binding.MpdivError) as e:
         binding.mpdiv_batch(big, dv[:1])
     assert e.value.code == binding.ERR_UNSUPPORTED
