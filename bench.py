@@ -492,7 +492,7 @@ def run_ours(args):
         "mpdiv_status": status,
         "step_ms_min_median_max": [float(np.min(ms)), float(np.median(ms)), float(np.max(ms))],
         "counters_one_step": {k: counters[k] for k in ("tiles", "mma_colsteps", "mma_products", "clipped_steps",
-                                                       "cluster_divs", "delta_pos", "delta_neg")},
+                                                       "chunks", "delta_pos", "delta_neg")},
         "version": binding.version(),
     }
     if not args.brief:
@@ -509,6 +509,36 @@ def run_ours(args):
                                        "div_per_s": 32 * 148 / (t15 * 1e-3), "frac_imad_pipe": f15[0],
                                        "frac_tensor_pipe": f15[1],
                                        "speedup_vs_printed_work": 32 * 148 / (t15 * 1e-3) * W_LIMB_PRODUCTS[1024] / peaks["imad_wide_chain"]}
+        del d15u, d15v, q15, r15
+        # 2^19-bit dividends (above the paper's shared-memory ceiling): the chunked form,
+        # the dividend streamed from HBM window by window
+        u19, v19 = inputs.uniform_operands(4 * 148, 16384, 8192, config=19)
+        d19u, d19v = to_dev(u19), to_dev(v19)
+        q19, r19 = torch.empty_like(d19u), torch.empty_like(d19v)
+        t19 = float(np.median(time_steps(lambda: binding.mpdiv_batch(d19u, d19v, q19, r19), 10, 3, flush)))
+        e19, c19, cnt19 = executed_work(binding, d19u, d19v, q19, r19)
+        f19 = pipe_fractions(e19, c19, t19, peaks)
+        out["range_extension_2^19_bits"] = {"batch": 4 * 148, "u_limbs": 16384, "v_limbs": 8192, "div_ms": t19,
+                                            "div_per_s": 4 * 148 / (t19 * 1e-3), "frac_imad_pipe": f19[0],
+                                            "frac_tensor_pipe": f19[1], "windows_per_division": cnt19["chunks"] / (4 * 148),
+                                            "note": "dividend not resident: quotient in windows of 2048 limbs, one "
+                                                    "shifted inverse of 2050 limbs for all windows (include/mpdiv.h)"}
+        del d19u, d19v, q19, r19
+        # small numbers in large batches -- one warp per division (32-thread blocks) against the
+        # 128-thread block per division that larger numbers use (forced with MPDIV_FLAG_THREADS)
+        small = {}
+        for ms_, ns_, bs_ in ((32, 16, 64 * 148), (128, 64, 64 * 148), (256, 128, 64 * 148), (512, 256, 32 * 148)):
+            us_, vs_ = inputs.uniform_operands(bs_, ms_, ns_, config=12)
+            dsu, dsv = to_dev(us_), to_dev(vs_)
+            qs, rs = torch.empty_like(dsu), torch.empty_like(dsv)
+            t_def = float(np.median(time_steps(lambda: binding.mpdiv_batch(dsu, dsv, qs, rs), 10, 3, flush)))
+            fl = binding.VARIANT_DEFAULT | binding.flag_threads(128)
+            t_blk = float(np.median(time_steps(lambda: binding.mpdiv_batch(dsu, dsv, qs, rs, variant=fl), 10, 3, flush)))
+            small["2^%d bits" % ((32 * ms_).bit_length() - 1)] = {
+                "batch": bs_, "u_limbs": ms_, "v_limbs": ns_, "div_per_s": bs_ / (t_def * 1e-3),
+                "div_per_s_128_thread_block_per_division": bs_ / (t_blk * 1e-3)}
+            del dsu, dsv, qs, rs
+        out["small_numbers_one_warp_per_division"] = small
         out["tensor_issue_probe"] = measure_mma_issue(binding)
         out["cpu_baseline"] = cpu_baseline(cfg)
         out["paper_context"] = "A100, 64-bit digits (PAPER.md:481-484): div/mul 6.77x/6.66x/6.94x/9.73x at 2^18..2^15 bits; model 5-7"

@@ -117,6 +117,8 @@ int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v
  *   MPDIV_FLAG_NO_HEAD     the head of Refine stays inside the division kernel (see mpdiv_batch_launches)
  *   MPDIV_FLAG_NO_MMA      every product of the division runs on the IMAD engine (no tcgen05 range products)
  *   MPDIV_FLAG_NO_CLUSTER  a small batch keeps one block per division (no thread-block cluster per division)
+ *   MPDIV_FLAG_CLUSTER(n)  clusters of at most n CTAs, n in {2, 4, 8}, wherever such clusters all run at once (default:
+ *                          at most 4, from 1024 limbs up, 2 only from 1536 limbs up)
  *   MPDIV_FLAG_THREADS(n)  block size override, n in {32, 64, 128, 256, 512}
  */
 #define MPDIV_VARIANT_PRINTED 0
@@ -129,6 +131,8 @@ int mpdiv_batch_noalloc(const uint32_t *u, int u_limbs, const uint32_t *v, int v
 #define MPDIV_FLAG_NO_CLUSTER 0x80
 #define MPDIV_FLAG_THREADS(n) ((n) == 64 ? 0x100 : (n) == 128 ? 0x200 : (n) == 256 ? 0x300 : (n) == 512 ? 0x400 : (n) == 32 ? 0x500 : 0)
 #define MPDIV_FLAG_THREADS_MASK 0x700
+#define MPDIV_FLAG_CLUSTER(n) ((n) == 2 ? 0x1000 : (n) == 4 ? 0x2000 : (n) == 8 ? 0x3000 : 0)
+#define MPDIV_FLAG_CLUSTER_MASK 0x3000
 int mpdiv_batch_ex(const uint32_t *u, int u_limbs, const uint32_t *v, int v_limbs,
                    uint32_t *q, uint32_t *r, int batch, int flags, mpdiv_stream_t stream);
 
@@ -278,7 +282,7 @@ int mpdiv_status(mpdiv_stream_t stream, unsigned int *flags, int reset);
  *          Refine from the 17-digit seed (mpdiv_seed_batch)
  *   out[16] tensor-core work: sum over range products of (MMA steps x accumulator columns); x 16384 = the
  *          u8 x u8 multiply-accumulates the tensor pipe executed (4 instructions of M = 128, K = 32 per step)
- *   out[17] reserved (0)      out[18] quotient windows of the chunked form (dividends above MPDIV_MAX_OPERAND_LIMBS
+ *   out[17] divisions that ran on a thread-block cluster      out[18] quotient windows of the chunked form (dividends above MPDIV_MAX_OPERAND_LIMBS
  *          limbs)      out[19..23] reserved (0)
  */
 #define MPDIV_NUM_COUNTERS 24

@@ -31,6 +31,11 @@ def flag_threads(n: int) -> int:
     """MPDIV_FLAG_THREADS(n): block size override."""
     return {32: 0x500, 64: 0x100, 128: 0x200, 256: 0x300, 512: 0x400}[int(n)]
 
+def flag_cluster(n: int) -> int:
+    """MPDIV_FLAG_CLUSTER(n): at most n CTAs per division in the cluster form."""
+    return {2: 0x1000, 4: 0x2000, 8: 0x3000}[int(n)]
+
+
 ENGINE_IMAD, ENGINE_TENSOR = 0, 1
 LINOP_ADD, LINOP_SUB, LINOP_NEG, LINOP_SHIFT, LINOP_PREC, LINOP_ANY = range(6)
 MAX_LIMBS = 16384          # u_limbs of mpdiv_batch (default variant)

@@ -39,9 +39,16 @@ enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT
        CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
        CNT_MMA_PRODUCTS, CNT_MMA_WAIT_FAILURES /* filled by the host from mp_mma.cuh */, CNT_SEED_ADDBACK, CNT_SEEDS,
        CNT_MMA_COLSTEPS, CNT_CLUSTER_DIVS, CNT_CHUNKS };
+__device__ __forceinline__ uint32_t cta_rank_in_cluster()
+{
+    uint32_t r;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// one count per division: the CTAs of a cluster (mp_mul.cuh) all run the same division, rank 0 counts
 __device__ __forceinline__ void count(int which, unsigned long long n = 1ull)
 {
-    if (threadIdx.x == 0) atomicAdd(&g_counters[which], n);
+    if (threadIdx.x == 0 && cta_rank_in_cluster() == 0) atomicAdd(&g_counters[which], n);
 }
 
 // Per-block bookkeeping for the scans/reductions: a double-buffered word per warp.
@@ -55,6 +62,7 @@ struct Blk {
     BlkScratch *sc;
     uint32_t parity;   // which half of sc->code the next collective uses
     uint32_t tiles;    // 8x8-limb tile products this thread has executed (debug counter)
+    uint32_t cl;       // cluster form (mp_mul.cuh): rank | size << 8 | staging set of the next product << 16; else 0
 };
 
 // ---------------------------------------------------------------------------------------

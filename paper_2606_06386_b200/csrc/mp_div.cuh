@@ -84,7 +84,7 @@ __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na,
 // the whole block (TT = T) or, for the early iterations whose operands are a few tiles long, warp 0 alone
 // (TT = 32: warp-level barriers only; the other warps wait at the block barrier that ends the narrow phase
 // and leave their issue slots to the other blocks of the SM).
-template <int TT, bool MMA = false>
+template <int TT, bool MMA = false, bool CL = false>
 __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it, int l, int wlen, limb *Wc, limb *Wn,
                                             limb *X, limb *P, const MulScratch &ms, Blk &blk, bool clip, MmaCtx *mma)
 {
@@ -106,7 +106,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
     int c = 0;                                             // X holds x / B^c
     if (L >= hpp) {
         // no room to truncate: full product and a comparison with B^h''
-        mul_full<TT>(Vp, pv, Wc, pw, P, ms, blk);
+        mul_full<TT, CL>(Vp, pv, Wc, pw, P, ms, blk);
         const int pl = round_up(pv, TILE) + round_up(pw, TILE);
         positive = !any_nonzero<TT>(P, hpp, pl);            // v'w < B^h''  (v'w != B^h'' here or x = 0)
         if (positive) {
@@ -123,7 +123,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         const int Klo2 = (clip && cx >= 25) ? (cx - 9) / 8 - 1 : 0;
         if (Klo2 <= 0) {
             // close product: only the L low limbs of v'w (MULTMOD)
-            mul_low<TT>(Vp, pv, Wc, pw, L, P, ms, blk);
+            mul_low<TT, CL>(Vp, pv, Wc, pw, L, P, ms, blk);
             positive = P[L - 1] != 0u;                     // top limb set: v'w just below B^h''
             xl = L;
             if (positive)
@@ -139,7 +139,7 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
                 count(CNT_MMA_PRODUCTS);
             } else {
                 c = TILE * Klo2;
-                mul_range<TT>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
+                mul_range<TT, CL>(Vp, pv, Wc, pw, Klo2, (L + TILE - 1) / TILE, P, ms, blk);
             }
             xl = L - c;
             positive = P[xl - 1] != 0u;
@@ -168,11 +168,11 @@ __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it,
         }
         if (tl >= 0) {
         } else if (Klo1 == 0) {
-            mul_full<TT>(Wc, pw, X, xl, P, ms, blk);
+            mul_full<TT, CL>(Wc, pw, X, xl, P, ms, blk);
             tl = round_up(pw, TILE) + round_up(xl, TILE);
             off = dd;
         } else {
-            tl = mul_range<TT>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
+            tl = mul_range<TT, CL>(Wc, pw, X, xl, Klo1, 1 << 20, P, ms, blk);
             off = dd - TILE * Klo1;
         }
         if (positive) {
@@ -330,7 +330,7 @@ __device__ __forceinline__ HeadPlan head_plan(int H, int iters)
 
 // w = Shinv(v, h) for B <= v (k = prec(v) - 1 >= 1), v zero padded to whole tiles above limb k.
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
-template <int T, bool MMA = false>
+template <int T, bool MMA = false, bool CL = false>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
                                            bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true,
                                            const limb *wmid = nullptr)
@@ -415,7 +415,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
                 __syncthreads();
                 blk.parity = 0;
             }
-            refine_step<T, MMA>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, mma);
+            refine_step<T, MMA, CL>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, mma);
         }
         l = l + m - 1;
         wlen = nlen;
@@ -447,6 +447,8 @@ __device__ __forceinline__ void shinv_head_warp(const limb *__restrict__ vg, int
     ms.HI = P + HEAD_P;
     ms.OV = ms.HI + HEAD_P;
     ms.C3 = ms.OV + HEAD_OV;
+    ms.ST = nullptr;
+    ms.stage_cap = 0;
     Blk blk{reinterpret_cast<BlkScratch *>(ms.C3 + HEAD_OV), 0u, 0u};
     // divisor prefix: limbs s_lo..k, s_lo the s of an iteration at l = HEAD_L (no head iteration reaches lower),
     // zeros above limb k

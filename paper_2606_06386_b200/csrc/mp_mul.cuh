@@ -191,7 +191,52 @@ struct MulScratch {
     limb *HI;
     uint32_t *OV;
     uint32_t *C3;
+    limb *ST;        // cluster form only: two staging sets of (LO | HI | OV), stage_cap limbs per LO and per HI
+    int stage_cap;
 };
+
+// ---------------------------------------------------------------------------------------
+// A thread-block CLUSTER per division (a batch smaller than the GPU leaves
+// most SMs idle and a lone block spends more than half of a 2^15-bit division in its tile diagonals).  Every CTA of the
+// cluster holds the whole state of the division and runs every linear operation itself -- those are latency bound
+// and gain nothing from more threads -- but a product's tile diagonals are dealt over ALL lanes of the cluster: a CTA
+// accumulates its share and writes each finished diagonal (LO | HI | OV) into the staging set of EVERY CTA through
+// distributed shared memory (mapa + st.shared::cluster), one cluster barrier makes the sets complete, and each CTA
+// resolves the carries from its own copy into its own product buffer.  The staging sets alternate between
+// products, so one barrier per product suffices: a CTA that is writing set s for product i + 2 has passed the barrier
+// of product i + 1, which every CTA reaches only after it has read set s of product i.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_size()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_map(uint32_t saddr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void cluster_st4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void cluster_st1(uint32_t addr, uint32_t a)
+{
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(a) : "memory");
+}
 
 // Phase 1: tile diagonals 0..Kd-1 of A (Na tiles) x Bp (Nb tiles) -> P (low 8 limbs of each
 // diagonal), HI, OV.  Operands must be 16-byte aligned and zero padded to whole tiles.
@@ -205,9 +250,11 @@ struct MulScratch {
 // T / 4 (cyclically: the up-ramp / plateau / down-ramp profile of a full product balances over the
 // passes; snake = true reverses odd passes, which balances the single ramp of a truncated product).
 // A pass that has fewer diagonals left than groups widens its groups (up to a whole warp).
-template <int T>
-__device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
-                                                  limb *P, limb *HI, uint32_t *OV, bool snake)
+// CL: the cluster form (above): crank / csize = this CTA's rank in its cluster and the cluster's size; P, HI, OV are the
+// staging set of this product.
+template <int T, bool CL>
+__device__ __forceinline__ uint32_t mul_diagonals_body(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                                       limb *P, limb *HI, uint32_t *OV, bool snake, int crank, int csize)
 {   // everything by value: a reference argument of a noinline function lives in local memory
     // lanes per diagonal: 4 for long diagonals, fewer when a diagonal has only a tile or two (the shuffle
     // reduction then costs more than it saves); a pass with spare threads widens its groups, but never
@@ -216,15 +263,20 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
     const int sh0 = maxlen <= 2 ? 0 : (maxlen <= 4 ? 1 : 2);
     int shmax = sh0;
     while (shmax < 5 && (2 << shmax) <= maxlen) ++shmax;
-    const int G0 = T >> sh0;                        // diagonals per full pass
+    const int TT = CL ? T * csize : T;              // lanes that share the product
+    const int G0 = TT >> sh0;                       // diagonals per full pass
     int pass = 0;
     uint32_t tiles = 0;
     for (int base = Klo; base < Kd; base += G0, ++pass) {
         const int ndiag = min(G0, Kd - base);
         int sh = sh0;
-        while (sh < shmax && (ndiag << (sh + 1)) <= T) ++sh;
+        while (sh < shmax && (ndiag << (sh + 1)) <= TT) ++sh;
         const int C = 1 << sh;
-        const int g = (int)threadIdx.x >> sh, c = (int)threadIdx.x & (C - 1);
+        // the groups of the cluster's CTAs interleave, so that neighbouring diagonals (similar lengths) go to different CTAs
+        // (giving a group a PAIR of diagonals of complementary lengths to level a single-ramp product was measured and
+        // lost 15 %: the fixed cost per diagonal -- first loads, finish, lane reduction, stores -- outweighs the balance)
+        const int g = CL ? ((int)threadIdx.x >> sh) * csize + crank : (int)threadIdx.x >> sh;
+        const int c = (int)threadIdx.x & (C - 1);
         const bool act = g < ndiag;
         const int K = base + ((snake && (pass & 1)) ? (ndiag - 1 - g) : g);
         const int Ilo = max(0, K - Nb + 1), Ihi = act ? min(Na - 1, K) : -1;
@@ -262,7 +314,21 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
             for (int i = 0; i < 17; i++) x[i] = __shfl_xor_sync(0xffffffffu, d[i], off);
             add17(d, x);
         }
-        if (act && c == 0) {
+        if (CL) {
+            if (act && c == 0) {                     // the finished diagonal goes to the staging set of every CTA
+                const uint32_t lp = (uint32_t)__cvta_generic_to_shared(P + TILE * K);
+                const uint32_t lh = (uint32_t)__cvta_generic_to_shared(HI + TILE * K);
+                const uint32_t lo = (uint32_t)__cvta_generic_to_shared(OV + K);
+                for (int rk = 0; rk < csize; ++rk) {
+                    const uint32_t rp = cluster_map(lp, (uint32_t)rk), rh = cluster_map(lh, (uint32_t)rk);
+                    cluster_st4(rp, d[0], d[1], d[2], d[3]);
+                    cluster_st4(rp + 16, d[4], d[5], d[6], d[7]);
+                    cluster_st4(rh, d[8], d[9], d[10], d[11]);
+                    cluster_st4(rh + 16, d[12], d[13], d[14], d[15]);
+                    cluster_st1(cluster_map(lo, (uint32_t)rk), d[16]);
+                }
+            }
+        } else if (act && c == 0) {
             uint4 *p4 = reinterpret_cast<uint4 *>(P + TILE * K);
             uint4 *h4 = reinterpret_cast<uint4 *>(HI + TILE * K);
             p4[0] = make_uint4(d[0], d[1], d[2], d[3]);
@@ -272,16 +338,31 @@ __device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb
             OV[K] = d[16];
         }
     }
-    grp_sync<T>();
+    if (CL) cluster_sync_all();
+    else grp_sync<T>();
     return tiles;
+}
+
+template <int T>
+__device__ __noinline__ uint32_t mul_diagonals(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                                  limb *P, limb *HI, uint32_t *OV, bool snake)
+{
+    return mul_diagonals_body<T, false>(A, Na, Bp, Nb, Klo, Kd, P, HI, OV, snake, 0, 1);
+}
+template <int T>
+__device__ __noinline__ uint32_t mul_diagonals_cluster(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                                       limb *P, limb *HI, uint32_t *OV, bool snake, int crank, int csize)
+{
+    return mul_diagonals_body<T, true>(A, Na, Bp, Nb, Klo, Kd, P, HI, OV, snake, crank, csize);
 }
 
 // Phase 2: resolve column blocks Klo..Kc-1 in place: P[K] = P[K] + HI[K-1] + OV[K-2] + carries,
 // where only diagonals Klo <= K < Kd contribute (nothing enters from below column block Klo).
 // Kc <= Kd + 2.  Ends with __syncthreads.
+// Pin: where the low halves of the diagonals are (P itself, or the staging set of the cluster form).
 template <int T>
-__device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, limb *HI, uint32_t *OV,
-                                                uint32_t *C3, Blk blk)
+__device__ __forceinline__ uint32_t mul_resolve_body(limb *P, const limb *Pin, int Klo, int Kd, int Kc, const limb *HI,
+                                                     const uint32_t *OV, uint32_t *C3, Blk blk)
 {   // blk by value (registers); the advanced collective parity is returned
     uint32_t cin = 0;
     for (int base = Klo; base < Kc; base += T) {
@@ -291,7 +372,7 @@ __device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, l
         uint32_t c3 = 0;
         if (active) {
             limb lo[8], hi[8];
-            if (K < Kd) load_tile(lo, P + TILE * K);
+            if (K < Kd) load_tile(lo, Pin + TILE * K);
             else {
 #pragma unroll
                 for (int j = 0; j < 8; j++) lo[j] = 0;
@@ -327,21 +408,57 @@ __device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, l
     return blk.parity;
 }
 
+template <int T>
+__device__ __noinline__ uint32_t mul_resolve(limb *P, int Klo, int Kd, int Kc, limb *HI, uint32_t *OV,
+                                                uint32_t *C3, Blk blk)
+{
+    return mul_resolve_body<T>(P, P, Klo, Kd, Kc, HI, OV, C3, blk);
+}
+template <int T>
+__device__ __noinline__ uint32_t mul_resolve_cluster(limb *P, const limb *Pin, int Klo, int Kd, int Kc, const limb *HI,
+                                                     const uint32_t *OV, uint32_t *C3, Blk blk)
+{
+    return mul_resolve_body<T>(P, Pin, Klo, Kd, Kc, HI, OV, C3, blk);
+}
+
+// words of one staging set: LO (cap) | HI (cap) | OV (one word per diagonal), cap a multiple of 32
+__host__ __device__ constexpr int stage_set_words(int cap) { return 2 * cap + cap / TILE + 4; }
+
+// The two phases of a product, block form or cluster form (CL).  Pd, HId, OVd, C3d are already offset so that index K
+// addresses diagonal K.  In the cluster form the diagonals pass through the staging set blk.cl selects.
+template <int T, bool CL>
+__device__ __forceinline__ void mul_phases(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd, int Kc, limb *Pd,
+                                           limb *HId, uint32_t *OVd, uint32_t *C3d, const MulScratch &ms, Blk &blk, bool snake)
+{
+    if constexpr (CL) {
+        const int cap = ms.stage_cap;
+        limb *S = ms.ST + ((blk.cl >> 16) & 1u) * (uint32_t)stage_set_words(cap);
+        limb *Ps = S - TILE * Klo, *HIs = S + cap - TILE * Klo;
+        uint32_t *OVs = S + 2 * cap - Klo;
+        blk.tiles += mul_diagonals_cluster<T>(A, Na, Bp, Nb, Klo, Kd, Ps, HIs, OVs, snake, (int)(blk.cl & 0xffu),
+                                              (int)((blk.cl >> 8) & 0xffu));
+        blk.parity = mul_resolve_cluster<T>(Pd, Ps, Klo, Kd, Kc, HIs, OVs, C3d, blk);
+        blk.cl ^= 1u << 16;
+    } else {
+        blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, snake);
+        blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
+    }
+}
+
 // P[0 .. 8*Kc) = (A * Bp) restricted to tile diagonals < Kd, carries resolved.
 //   full product      : Kd = Na + Nb - 1 (or more), Kc = Na + Nb
 //   product mod B^L   : Kd = Kc = ceil(L / 8); limbs >= L of the last block are not meaningful
 // na, nb in limbs; operands zero padded to whole tiles.
-template <int T>
+template <int T, bool CL = false>
 __device__ __forceinline__ void mul_full(const limb *A, int na, const limb *Bp, int nb, limb *P,
                                          const MulScratch &ms, Blk &blk)
 {
     const int Na = (na + TILE - 1) / TILE, Nb = (nb + TILE - 1) / TILE;
     const int Kd = Na + Nb - 1;
-    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, false);
-    blk.parity = mul_resolve<T>(P, 0, Kd, Na + Nb, ms.HI, ms.OV, ms.C3, blk);
+    mul_phases<T, CL>(A, Na, Bp, Nb, 0, Kd, Na + Nb, P, ms.HI, ms.OV, ms.C3, ms, blk, false);
 }
 
-template <int T>
+template <int T, bool CL = false>
 __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, int nb, int L, limb *P,
                                         const MulScratch &ms, Blk &blk)
 {
@@ -349,8 +466,7 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
     const int Kfull = Na + Nb;
     const int Kc = min((L + TILE - 1) / TILE, Kfull);
     const int Kd = min(Kc, Kfull - 1);
-    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, 0, Kd, P, ms.HI, ms.OV, Kd < Kfull - 1);
-    blk.parity = mul_resolve<T>(P, 0, Kd, Kc, ms.HI, ms.OV, ms.C3, blk);
+    mul_phases<T, CL>(A, Na, Bp, Nb, 0, Kd, Kc, P, ms.HI, ms.OV, ms.C3, ms, blk, Kd < Kfull - 1);
 }
 
 // Clipped ("range") product: only tile diagonals Klo <= K < Khi are computed, so the result is
@@ -359,7 +475,7 @@ __device__ __forceinline__ void mul_low(const limb *A, int na, const limb *Bp, i
 // columns end at 8*Klo + 6).  The block stores limb 8*Klo + i of that value at P[i] -- the buffers
 // only need 8*(Khi - Klo) limbs -- and limbs below 8*Klo are not produced.  Khi is clamped to the
 // size of the full product.  Returns the number of limbs stored.
-template <int T>
+template <int T, bool CL = false>
 __device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, int nb, int Klo, int Khi,
                                          limb *P, const MulScratch &ms, Blk &blk)
 {
@@ -369,8 +485,7 @@ __device__ __forceinline__ int mul_range(const limb *A, int na, const limb *Bp, 
     const int Kd = min(Kc, Kfull - 1);
     limb *Pd = P - TILE * Klo, *HId = ms.HI - TILE * Klo;
     uint32_t *OVd = ms.OV - Klo, *C3d = ms.C3 - Klo;
-    blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, true);
-    blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
+    mul_phases<T, CL>(A, Na, Bp, Nb, Klo, Kd, Kc, Pd, HId, OVd, C3d, ms, blk, true);
     return TILE * max(Kc - Klo, 0);
 }
 

@@ -88,7 +88,7 @@ mpmul_kernel(const limb *__restrict__ a, int a_limbs, const limb *__restrict__ b
 {
     extern __shared__ __align__(1024) uint32_t smem[];
     limb *A = smem + L.a_off, *Bs = smem + L.b_off, *P = smem + L.p_off;
-    MulScratch ms{smem + L.hi_off, smem + L.ov_off, smem + L.c3_off};
+    MulScratch ms{smem + L.hi_off, smem + L.ov_off, smem + L.c3_off, nullptr, 0};
     Blk blk{reinterpret_cast<BlkScratch *>(smem + L.sc_off), 0u};
     MmaCtx mcx;
     bool tensor = false;
@@ -224,6 +224,8 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 // Tuning switches carried by the `flags` argument of the *_ex calls (include/mpdiv.h).
 struct Tune {
     bool no_seed, no_head, no_mma, no_cluster;
+    int cluster_cap;                             // largest cluster per division (MPDIV_FLAG_CLUSTER; default 4)
+    bool cluster_forced;                         // MPDIV_FLAG_CLUSTER given: use clusters wherever they fit
     int threads;                                 // 0 = by size
     limb *wmid_fixed;                            // mpdiv_batch_noalloc: the head kernel's rows live here (no pool allocation)
 };
@@ -234,6 +236,9 @@ Tune tune_of(int flags)
     t.no_head = (flags & MPDIV_FLAG_NO_HEAD) != 0;
     t.no_mma = (flags & MPDIV_FLAG_NO_MMA) != 0;
     t.no_cluster = (flags & MPDIV_FLAG_NO_CLUSTER) != 0;
+    const int cc = (flags & MPDIV_FLAG_CLUSTER_MASK) >> 12;
+    t.cluster_cap = cc ? 1 << cc : 4;
+    t.cluster_forced = cc != 0;
     const int c = (flags & MPDIV_FLAG_THREADS_MASK) >> 8;
     t.threads = c >= 1 && c <= 4 ? 32 << c : (c == 5 ? 32 : 0);
     t.wmid_fixed = nullptr;
@@ -244,7 +249,7 @@ bool flags_ok(int flags)
     const int var = flags & MPDIV_VARIANT_MASK;
     if (var != MPDIV_VARIANT_PRINTED && var != MPDIV_VARIANT_CLIPPED) return false;
     if (flags & ~(MPDIV_VARIANT_MASK | MPDIV_FLAG_NO_SEED | MPDIV_FLAG_NO_HEAD | MPDIV_FLAG_NO_MMA | MPDIV_FLAG_NO_CLUSTER |
-                  MPDIV_FLAG_THREADS_MASK)) return false;
+                  MPDIV_FLAG_THREADS_MASK | MPDIV_FLAG_CLUSTER_MASK)) return false;
     return ((flags & MPDIV_FLAG_THREADS_MASK) >> 8) <= 5;
 }
 

@@ -16,6 +16,8 @@ struct DivLayout {
     int p_words_q;    // quotient phase: capacity of P and of HI
     int hcap;         // the layout holds instances with H = max(h - k, 2) <= hcap
     int qb_off;       // chunked form (mpdiv_kernel<.., BIG>): the quotient chunk's own buffer; otherwise = wa_off
+    int stage_off;    // cluster form (mpdiv_kernel<.., CL>): two staging sets of stage_set_words(stage_cap) words, or -1
+    int stage_cap;
 };
 
 // M: limbs of the dividend side (u stride, or h for shinv_batch); n: divisor stride;
@@ -57,7 +59,19 @@ static DivLayout div_layout(int M, int n, bool with_quotient, bool clip, int hca
     L.mma_cols = 0;
     L.hcap = hc;
     L.qb_off = L.wa_off;
+    L.stage_off = -1;
+    L.stage_cap = 0;
     return L;
+}
+
+// Adds the staging sets of the cluster form (mp_mul.cuh) behind layout L; returns the bytes.
+static size_t div_layout_add_stage(DivLayout &L)
+{
+    const int pw = L.p_words_r > L.p_words_q ? L.p_words_r : L.p_words_q;
+    L.stage_cap = round_up(pw + 2 * TILE, 32);
+    L.stage_off = round_up(L.total_words, 4);
+    L.total_words = L.stage_off + 2 * stage_set_words(L.stage_cap);
+    return (size_t)L.total_words * 4;
 }
 
 // H up to which an instance takes the compact layout: the configs' shape H = M/2 + 1 with room to spare.
@@ -157,6 +171,8 @@ __device__ __forceinline__ ShinvBufs refine_bufs(uint32_t *smem, const DivLayout
     b.ms.HI = b.P + L.p_words_r;
     b.ms.OV = b.ms.HI + L.p_words_r;
     b.ms.C3 = b.ms.OV + ov;
+    b.ms.ST = L.stage_off >= 0 ? smem + L.stage_off : nullptr;
+    b.ms.stage_cap = L.stage_cap;
     return b;
 }
 
@@ -319,7 +335,9 @@ __device__ __forceinline__ void copy_row_global(limb *__restrict__ dst, const li
 // x_c < v B^t, so its quotient has t limbs, and ONE inverse w = Shinv(v, k + 1 + t) serves every window
 // (q0 = floor(x w / B^(k+1+t)) is within the range of the bounded correction loops for any x < B^(k+1+t)).
 // A division with D <= t is a single window with h_w = h: exactly the resident algorithm.
-template <int T, bool LAT, bool MMA, bool BIG = false>
+// CL = the cluster form (mp_mul.cuh): the CTAs of a thread-block cluster all run the division of instance
+// %clusterid.x on their own copy of the state and share the tile diagonals of every product; rank 0 stores.
+template <int T, bool LAT, bool MMA, bool BIG = false, bool CL = false>
 __global__ void __launch_bounds__(T, LAT ? (T <= 128 ? 2 : 1) : 512 / T)
 mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
              limb *__restrict__ q, limb *__restrict__ r, int batch, DivLayout L, DivLayout Lc, int clip, int narrow_l,
@@ -335,6 +353,14 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     const int vpad = round_up(v_limbs, TILE) + 16, upad = round_up(u_limbs, TILE) + 16;
     static_assert(!MMA || DivMma<T, LAT>::value, "no tensor-core engine for this block size");
     static_assert(!BIG || !LAT, "the chunked form is a throughput kernel");
+    static_assert(!CL || (LAT && !MMA && !BIG), "the cluster form is a latency kernel on the IMAD engine");
+    uint32_t crank = 0, inst0 = blockIdx.x, inst_step = gridDim.x;
+    if constexpr (CL) {
+        crank = cluster_rank();
+        blk.cl = crank | (cluster_size() << 8);
+        asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(inst0));
+        asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(inst_step));
+    }
     MmaCtx mcx;
     MmaCtx *mma = nullptr;
     if constexpr (MMA) {
@@ -348,8 +374,9 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
     }
     IoBar io;
     io_init<T>(io, blk.sc);
+    if constexpr (CL) cluster_sync_all();                  // every CTA of the cluster is running before any remote store
 
-    for (int inst = blockIdx.x; inst < batch; inst += gridDim.x) {
+    for (int inst = (int)inst0; inst < batch; inst += (int)inst_step) {
         const limb *ug = u + (size_t)inst * u_limbs;
         const limb *vg = v + (size_t)inst * v_limbs;
         limb *qg = q + (size_t)inst * u_limbs;
@@ -370,17 +397,21 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         if (pv == 0) {                                     // v = 0: q = all ones, r = low limbs of u
             count(CNT_V_ZERO);
             raise_status(ST_V_ZERO);
-            for (int i = threadIdx.x; i < u_limbs; i += T) qg[i] = 0xffffffffu;
-            if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, min(u_limbs, v_limbs));
-            else store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
+            if (crank == 0) {
+                for (int i = threadIdx.x; i < u_limbs; i += T) qg[i] = 0xffffffffu;
+                if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, min(u_limbs, v_limbs));
+                else store_number<T>(rg, U + 4, v_limbs, min(u_limbs, v_limbs));
+            }
             __syncthreads();
             continue;
         }
         if (pv > h) {                                      // u < v: (0, u)
             count(CNT_U_LT_V);
-            store_row<T>(qg, U + 4, u_limbs, 0);
-            if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, h);
-            else store_number<T>(rg, U + 4, v_limbs, h);
+            if (crank == 0) {
+                store_row<T>(qg, U + 4, u_limbs, 0);
+                if constexpr (BIG) copy_row_global<T>(rg, ug, v_limbs, h);
+                else store_number<T>(rg, U + 4, v_limbs, h);
+            }
             __syncthreads();
             continue;
         }
@@ -413,6 +444,8 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         mq.HI = PQ + Li.p_words_q;
         mq.OV = mq.HI + Li.p_words_q;
         mq.C3 = mq.OV + round_up(Li.p_words_q / TILE, 4);
+        mq.ST = rb.ms.ST;
+        mq.stage_cap = rb.ms.stage_cap;
 
         // chunks of the quotient (BIG; otherwise one window = the whole dividend)
         const int D = h - k;                               // q < B^D
@@ -420,7 +453,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         const int hx = (BIG && nchunks > 1) ? k + 1 + tchunk : h;     // every window is < B^hx
 
         // a3..a8: shifted inverse (U area is reused as the second iterate buffer)
-        const int nw = shinv_block<T, MMA>(Vb, k, hx, rb, blk, clip != 0, mma_i, narrow_l & 255, !(narrow_l & 256),
+        const int nw = shinv_block<T, MMA, CL>(Vb, k, hx, rb, blk, clip != 0, mma_i, narrow_l & 255, !(narrow_l & 256),
                                       (wmid && !one_limb) ? wmid + (size_t)inst * WMID_STRIDE : nullptr);
         const int psh = top_prec(WA, nw);
 
@@ -469,7 +502,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             if (psh == 0) {
                 lin_zero<T>(Q, qlen);
             } else {
-                mul_full<T>(Ub, h, WA, psh, PQ, mq, blk);
+                mul_full<T, CL>(Ub, h, WA, psh, PQ, mq, blk);
                 const int pl = round_up(h, TILE) + round_up(psh, TILE);
                 lin_copy<T>(Q, qlen, PQ, pl, h);           // WA (shinv) is dead: reuse it for q
             }
@@ -479,7 +512,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             rlen = round_up(h + 1, TILE);                  // p <= u + v < 2 B^h
             int pl = 0;
             if (pq > 0) {
-                mul_full<T>(Vb, k + 1, Q, pq, PQ, mq, blk);
+                mul_full<T, CL>(Vb, k + 1, Q, pq, PQ, mq, blk);
                 pl = round_up(k + 1, TILE) + round_up(pq, TILE);
             }
 
@@ -503,7 +536,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                     lin_copy<T>(Q, qlen, PQ, pl, hx - 32 * dlo);
                 } else {
                     const int Klo = (hx >= 17) ? (hx - 9) / TILE : 0;
-                    pl = mul_range<T>(Ub, hx, WA, psh, Klo, 1 << 20, PQ, mq, blk);
+                    pl = mul_range<T, CL>(Ub, hx, WA, psh, Klo, 1 << 20, PQ, mq, blk);
                     lin_copy<T>(Q, qlen, PQ, pl, hx - TILE * Klo);
                 }
             }
@@ -518,7 +551,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
                     count(CNT_MMA_PRODUCTS);
                     pl = min(rlen, pl);
                 } else {
-                    mul_low<T>(Vb, k + 1, Q, pq, rlen, PQ, mq, blk);
+                    mul_low<T, CL>(Vb, k + 1, Q, pq, rlen, PQ, mq, blk);
                     pl = min(rlen, round_up(k + 1, TILE) + round_up(pq, TILE));
                 }
             }
@@ -560,14 +593,17 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             }
             count(CNT_CHUNKS);
             __syncthreads();
-        } else {
+        } else if (crank == 0) {
             store_row<T>(qg, Q, u_limbs, min(qlen, u_limbs));
         }
         }   // chunks
 
         // a12: the remainder (of the scaled problem it is r*B for one-limb divisors)
-        if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
-        else store_row<T>(rg, R, v_limbs, min(round_up(k + 1, 4), v_limbs));
+        if (crank == 0) {
+            if (one_limb) store_number<T>(rg, R + 1, v_limbs, 1);
+            else store_row<T>(rg, R, v_limbs, min(round_up(k + 1, 4), v_limbs));
+        }
+        if constexpr (CL) count(CNT_CLUSTER_DIVS);
         __syncthreads();
     }
     count_tiles(blk);
@@ -663,10 +699,77 @@ static cudaMemPool_t head_pool()
     return pools[dev];
 }
 
+// A thread-block cluster per division (mpdiv_kernel<128, true, false, false, true>): for batches so small that
+// clusters of `cs` CTAs still run all at once.  Returns the largest admissible size in {8, 4, 2} (at most cap), or 1.
+static int cluster_size_for(int batch, int cap, size_t bytes)
+{
+    for (int cs = 8; cs >= 2; cs /= 2) {
+        if (cs > cap || batch * cs > g_sm_count) continue;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(batch * cs));
+        cfg.blockDim = dim3(128);
+        cfg.dynamicSmemBytes = bytes;
+        cudaLaunchAttribute at;
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = (unsigned)cs;
+        at.val.clusterDim.y = 1;
+        at.val.clusterDim.z = 1;
+        cfg.attrs = &at;
+        cfg.numAttrs = 1;
+        int nact = 0;
+        if (cudaOccupancyMaxActiveClusters(&nact, mpdiv_kernel<128, true, false, false, true>, &cfg) != cudaSuccess) {
+            cudaGetLastError();
+            continue;
+        }
+        if (nact >= batch) return cs;
+    }
+    return 1;
+}
+
+static int launch_div_cluster(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
+                              cudaStream_t st, int clip, const Tune &tn)
+{
+    DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
+    const size_t bytes = div_layout_add_stage(L);
+    if ((int)bytes > g_max_smem) return -1;
+    if (set_smem(mpdiv_kernel<128, true, false, false, true>, bytes) != MPDIV_OK) return -1;
+    const int cs = cluster_size_for(batch, tn.cluster_cap, bytes);
+    if (cs < 2 || (cs == 2 && !tn.cluster_forced && u_limbs < 1536)) return -1;   // two CTAs do not pay below 2^16 bits
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(batch * cs));
+    cfg.blockDim = dim3(128);
+    cfg.dynamicSmemBytes = bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute at;
+    at.id = cudaLaunchAttributeClusterDimension;
+    at.val.clusterDim.x = (unsigned)cs;
+    at.val.clusterDim.y = 1;
+    at.val.clusterDim.z = 1;
+    cfg.attrs = &at;
+    cfg.numAttrs = 1;
+    const limb *wmid = nullptr;
+    const int narrow = tn.no_seed ? 256 : 0;                 // never the narrow mode: every thread takes part in every product
+    if (cudaLaunchKernelEx(&cfg, mpdiv_kernel<128, true, false, false, true>, u, u_limbs, v, v_limbs, q, r, batch, L, L, clip,
+                           narrow, wmid, 0) != cudaSuccess) {
+        cudaGetLastError();
+        return MPDIV_ERR_CUDA;
+    }
+    return MPDIV_OK;
+}
+
 template <int T, bool LAT, bool MMA>
 int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
                  cudaStream_t st, int clip, int sched, bool tensor, const Tune &tn)
 {
+    if constexpr (T == 128 && LAT && !MMA) {
+        // a batch that leaves most SMs idle: a cluster of CTAs per division shares the tile diagonals of every product
+        // (measured, 32 divisions: 2^16 bits 121 -> 99 us on four CTAs, 105 us on two; 2^15 bits 73 us either way on four,
+        // 75 us on two; 2^14 bits 56 -> 60 us: the cluster barrier and the remote stores cost ~700 cycles per product)
+        if (!tn.no_cluster && tn.threads == 0 && 2 * batch <= g_sm_count && (u_limbs >= 1024 || tn.cluster_forced)) {
+            const int rc = launch_div_cluster(u, u_limbs, v, v_limbs, q, r, batch, st, clip, tn);
+            if (rc >= 0) return rc;
+        }
+    }
     DivLayout L = div_layout(u_limbs + 1, v_limbs, true, clip != 0);
     DivLayout Lc = L;                                        // Lc.mma_off < 0: no engine, Lc unused
     size_t bytes = (size_t)L.total_words * 4;

@@ -45,7 +45,7 @@ def test_bad_arguments_rejected_before_any_cuda_call():
     assert lib.mpdiv_batch(p, 8, p, 4, p, p, 0, null) == binding.ERR_BAD_ARG          # empty batch
     assert lib.mpdiv_batch(p + 4, 8, p, 4, p, p, 1, null) == binding.ERR_BAD_ARG      # misaligned
     assert lib.mpdiv_batch_ex(p, 8, p, 4, p, p, 1, 7, null) == binding.ERR_BAD_ARG    # unknown variant
-    assert lib.mpdiv_batch_ex(p, 8, p, 4, p, p, 1, 0x1000, null) == binding.ERR_BAD_ARG   # unknown flag bit
+    assert lib.mpdiv_batch_ex(p, 8, p, 4, p, p, 1, 0x4000, null) == binding.ERR_BAD_ARG   # unknown flag bit
     assert lib.mpdiv_batch(p, 8, p, 8196, p, p, 1, null) == binding.ERR_UNSUPPORTED    # v stride above the maximum
     assert lib.mpdiv_batch(p, 16388, p, 4, p, p, 1, null) == binding.ERR_UNSUPPORTED   # u stride above the maximum
     assert lib.mpmul_batch(p, 8, p, 8, p, 20, 1, null) == binding.ERR_BAD_ARG         # c_limbs > a+b
