@@ -63,11 +63,16 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 // global -> shared, completion counted in bytes on the mbarrier (a CTA-local shared address is a valid shared::cluster
-// address of the executing CTA)
-__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar)
+// address of the executing CTA), with an L2 eviction priority for the row: a row that is fetched again later in the
+// kernel (u, whose shared-memory words serve Refine as an iterate buffer in between) is kept in L2, a row read for the
+// last time is not
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar, bool keep)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+    uint64_t pol;
+    if (keep) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(dst_smem), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
 }
 // shared -> global, tracked by the issuing thread's bulk groups
 __device__ __forceinline__ void bulk_s2g(void *dst, uint32_t src_smem, uint32_t bytes)
@@ -83,15 +88,16 @@ __device__ __forceinline__ void bulk_commit_wait()
 // Up to two rows HBM -> shared memory by bulk copy: d_i[0..n_i) = s_i[0..n_i), d_i[n_i..pad_i) = 0 (n_i a multiple of 4,
 // n_1 = 0 for a single row).  The destinations must not be in use by any thread (the caller's last block barrier is
 // behind every earlier access); on return both rows and their padding are visible to the whole block.
+// keep1: row 1 will be fetched again by this block (L2 evict_last); every other row is read for the last time.
 template <int T>
 __device__ __forceinline__ void load_rows(IoBar &io, limb *d0, const limb *__restrict__ s0, int n0, int pad0,
-                                          limb *d1, const limb *__restrict__ s1, int n1, int pad1)
+                                          limb *d1, const limb *__restrict__ s1, int n1, int pad1, bool keep1 = false)
 {
     if (threadIdx.x == 0) {
         fence_async_smem();                                  // earlier generic-proxy accesses of the destinations
         mbar_expect_tx(io.bar, 4u * (uint32_t)(n0 + n1));
-        bulk_g2s(smem_u32(d0), s0, 4u * (uint32_t)n0, io.bar);
-        if (n1 > 0) bulk_g2s(smem_u32(d1), s1, 4u * (uint32_t)n1, io.bar);
+        bulk_g2s_hint(smem_u32(d0), s0, 4u * (uint32_t)n0, io.bar, false);
+        if (n1 > 0) bulk_g2s_hint(smem_u32(d1), s1, 4u * (uint32_t)n1, io.bar, keep1);
     }
     for (int i = n0 + (int)threadIdx.x; i < pad0; i += T) d0[i] = 0u;
     for (int i = n1 + (int)threadIdx.x; i < pad1; i += T) d1[i] = 0u;

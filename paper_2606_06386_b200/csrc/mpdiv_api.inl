@@ -389,7 +389,7 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
             load_rows<T>(io, V + 4, vg, v_limbs, vpad - 4, nullptr, nullptr, 0, 0);
             h = global_prec<T>(ug, u_limbs, blk);
         } else {
-            load_rows<T>(io, V + 4, vg, v_limbs, vpad - 4, U + 4, ug, u_limbs, upad - 4);
+            load_rows<T>(io, V + 4, vg, v_limbs, vpad - 4, U + 4, ug, u_limbs, upad - 4, true);   // u comes back after Refine
             h = prec_of<T>(U + 4, u_limbs, blk);
         }
         const int pv = prec_of<T>(V + 4, v_limbs, blk);
