@@ -288,7 +288,7 @@ def config_row(binding, cfg, flush, peaks):
     med = lambda fn: float(np.median(time_steps(fn, 25, 3, flush)))   # noqa: E731
     t_div = med(lambda: binding.mpdiv_batch(du, dv, q, r))
     t_div_printed = med(lambda: binding.mpdiv_batch(du, dv, q, r, variant=binding.VARIANT_PRINTED))
-    ex_imad, ex_tc, _ = executed_work(binding, du, dv, q, r)
+    ex_imad, ex_tc, cnt_row = executed_work(binding, du, dv, q, r)
     exp_imad, exp_tc, _ = executed_work(binding, du, dv, q, r, variant=binding.VARIANT_PRINTED)
     f_imad, f_tc, bound = pipe_fractions(ex_imad, ex_tc, t_div, peaks)
     # R1 unit: M x M -> low M limbs (the paper's "full multiplication", M^2/2 limb products);
@@ -318,6 +318,7 @@ def config_row(binding, cfg, flush, peaks):
         "div_ms": t_div, "div_per_s": b / (t_div * 1e-3), "us_per_div_latency": t_div * 1e3 if b <= 148 else None,
         "frac_imad_pipe": f_imad, "frac_tensor_pipe": f_tc, "bound": bound, "frac": max(f_imad, f_tc),
         "executed_limb_products_per_div": ex_imad / b, "executed_tensor_macs_per_div": ex_tc / b,
+        "tensor_unit_occupancy": cnt_row["mma_unit_cycles"] / (peaks["sm_count"] * t_div * 1e-3 * peaks["sm_hz"]),
         "printed_div_per_s": b / (t_div_printed * 1e-3),
         "frac_printed": exp_imad / (t_div_printed * 1e-3) / peaks["imad_wide_chain"],
         "mul_MxM_lowM_ms": {"imad": t_m1, "tensor": t_m1_tc}, "mul_nxn_full_ms": {"imad": t_m2, "tensor": t_m2_tc},
@@ -436,6 +437,8 @@ def run_ours(args):
     peaks = measure_imad_peak(binding)
     peaks["tensor_u8_mac"] = measure_tensor_peak(binding)
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    peaks["sm_count"] = sm_count
+    peaks["sm_hz"] = (clocks.get("sm_mhz") or 1965.0) * 1e6
     kernel_ms = float(np.mean(ms))
     ex_imad, ex_tc, counters = executed_work(binding, du, dv, q, r)
     f_imad, f_tc, bound = pipe_fractions(ex_imad, ex_tc, kernel_ms, peaks)
@@ -453,6 +456,10 @@ def run_ours(args):
         "frac_imad_pipe": f_imad, "frac_tensor_pipe": f_tc,
         "executed_limb_products_per_launch": ex_imad, "executed_tensor_macs_per_launch": ex_tc,
         "peak_imad_limb_products_per_s": peaks["imad_wide_chain"], "peak_tensor_u8_macs_per_s": peaks["tensor_u8_mac"],
+        # how long the tensor unit is OCCUPIED (not how much arithmetic it does): the Toeplitz operand is read from
+        # shared memory, so an instruction of N columns holds the unit max(32 + N/4, N/2) cycles (mpdiv_mma_probe form
+        # 1), N/2 of them multiplying; counted per issued instruction by the engine, over all SMs at the clock seen
+        "tensor_unit_occupancy": counters["mma_unit_cycles"] / (sm_count * kernel_ms * 1e-3 * peaks["sm_hz"]),
         "peak_source": "measured in this run: mpdiv_imad_probe kind 0 (carry-chained IMAD.WIDE.U32 tile, no memory; "
                        "nominal 32/clk/SM) and mpdiv_mma_probe (tcgen05.mma.kind::i8 M=128 N=128 K=32 from two warps, "
                        "events; nominal 8192 MAC/clk/SM)",

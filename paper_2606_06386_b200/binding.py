@@ -289,7 +289,7 @@ def mma_probe(n_cols: int, issuers: int = 1, iters: int = 2000, form: int = 0, s
 
 COUNTER_NAMES = ("delta_neg", "delta_pos", "delta_multi", "one_limb", "u_lt_v", "v_zero", "sign_neg", "pow_b",
                  "tiles", "delta_neg_multi", "delta_out_of_range", "clipped_steps", "mma_products", "mma_wait_failures",
-                 "seed_addbacks", "seeds", "mma_colsteps", "cluster_divs", "chunks")
+                 "seed_addbacks", "seeds", "mma_colsteps", "cluster_divs", "chunks", "mma_unit_cycles")
 
 
 def debug_counters(reset: bool = False, stream=None) -> dict:

@@ -38,7 +38,7 @@ __device__ unsigned long long g_counters[NUM_COUNTERS];
 enum { CNT_DELTA_NEG = 0, CNT_DELTA_POS, CNT_DELTA_MULTI, CNT_ONE_LIMB, CNT_U_LT_V, CNT_V_ZERO,
        CNT_SIGN_NEG, CNT_POW_B, CNT_TILES, CNT_DELTA_NEG_MULTI, CNT_DELTA_OUT_OF_RANGE, CNT_CLIPPED_STEPS,
        CNT_MMA_PRODUCTS, CNT_MMA_WAIT_FAILURES /* filled by the host from mp_mma.cuh */, CNT_SEED_ADDBACK, CNT_SEEDS,
-       CNT_MMA_COLSTEPS, CNT_CLUSTER_DIVS, CNT_CHUNKS };
+       CNT_MMA_COLSTEPS, CNT_CLUSTER_DIVS, CNT_CHUNKS, CNT_MMA_UNIT_CYCLES };
 __device__ __forceinline__ uint32_t cta_rank_in_cluster()
 {
     uint32_t r;

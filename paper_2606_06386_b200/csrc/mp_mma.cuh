@@ -481,6 +481,15 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     cx_mem.empty_par = cx.empty_par;
     cx_mem.ndone = cx.ndone;
     count(CNT_MMA_COLSTEPS, (unsigned long long)nsteps * (unsigned long long)Nn);   // x 16384 = u8 MACs executed
+    {   // cycles the tensor unit is occupied by this product's instructions: 4 per step and 256-column chunk, each
+        // max(32 + n/4, n/2) -- the Toeplitz tile comes from shared memory (128 rows x 32 bytes = 32 cycles), see the header
+        unsigned long long cyc = 0;
+        for (int nc = 0; nc < Nn; nc += 256) {
+            const int n = min(256, Nn - nc);
+            cyc += 4ull * (unsigned long long)max(32 + n / 4, n / 2);
+        }
+        count(CNT_MMA_UNIT_CYCLES, cyc * (unsigned long long)nsteps);
+    }
     return 32 * N;
 }
 

@@ -15,7 +15,7 @@
 
 using namespace mpd;
 
-#define MPDIV_VERSION_STR "mpdiv 0.6 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products"
+#define MPDIV_VERSION_STR "mpdiv 0.7 sm_100a (B200) limbs=u32 imad.wide 8x8 tiles + int8 tcgen05 range products, bulk-copy rows, warp/block/cluster per division, dividends to 2^19 bits"
 
 // ---------------------------------------------------------------------------------------
 // mpmul_batch
