@@ -985,12 +985,14 @@ int mpdiv_batch_host(const uint32_t *u_host, int u_limbs, const uint32_t *v_host
     uint32_t *dq = dv + (size_t)batch * v_limbs;
     uint32_t *dr = dq + (size_t)batch * u_limbs;
 
-    // Chunks of one division per SM (at most MAXC of them).  The upload of chunk i+1 and the download of chunk
+    // Chunks of one division per SM, two up to 2048 limbs (at most MAXC chunks).  The upload of chunk i+1 and the download of chunk
     // i-1 overlap the division of chunk i, and the chunk kernels go round NK streams so that the blocks of
     // consecutive chunks share the SMs like the blocks of one launch would (a chunk alone would leave each SM
     // with a single block); the kernel flavour is the one the whole batch would get.
     constexpr int MAXC = 16, NK = 4;
-    int nchunks = batch / g_sm_count;
+    // (measured at config 2: 4 chunks 590 us, 8 chunks 620-640 us, 2 chunks 640 us, 1 chunk 850 us per batch; at configs 3 and
+    // 4, whose kernels take as long as their copies, one division per SM and chunk is 7-10 % faster than two)
+    int nchunks = batch / ((u_limbs <= 2048 ? 2 : 1) * g_sm_count);
     if (nchunks < 1) nchunks = 1;
     if (nchunks > MAXC) nchunks = MAXC;
     const int chunk = (batch + nchunks - 1) / nchunks;
