@@ -68,14 +68,14 @@ struct MmaEnabled { static constexpr bool value = (T == 512 || T == 256 || T == 
 // Range product on the tensor core when the plan says it wins, else -1 (caller runs the IMAD path).
 // P[i] = limb 32*dlo + i.
 template <int T, bool MMA = MmaEnabled<T>::value>
-__device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na, const limb *Bp, int nb, int dlo, int dhi,
+__device__ __forceinline__ int try_mma_range(const MmaRef &mma, const limb *A, int na, const limb *Bp, int nb, int dlo, int dhi,
                                              limb *P, limb *HI, Blk &blk)
 {
     if constexpr (MMA) {
         bool swap;
         if (mma_plan<T>(mma, na, nb, dlo, dhi, swap))
-            return swap ? mma_mul_range<T>(*mma, Bp, nb, A, na, dlo, dhi, P, HI, blk)
-                        : mma_mul_range<T>(*mma, A, na, Bp, nb, dlo, dhi, P, HI, blk);
+            return swap ? mma_mul_range<T>(*mma.cx, Bp, nb, A, na, dlo, dhi, P, HI, blk)
+                        : mma_mul_range<T>(*mma.cx, A, na, Bp, nb, dlo, dhi, P, HI, blk);
     }
     return -1;
 }
@@ -86,7 +86,7 @@ __device__ __forceinline__ int try_mma_range(MmaCtx *mma, const limb *A, int na,
 // and leave their issue slots to the other blocks of the SM).
 template <int TT, bool MMA = false, bool CL = false>
 __device__ __forceinline__ void refine_step(const limb *V, int k, int H, int it, int l, int wlen, limb *Wc, limb *Wn,
-                                            limb *X, limb *P, const MulScratch &ms, Blk &blk, bool clip, MmaCtx *mma)
+                                            limb *X, limb *P, const MulScratch &ms, Blk &blk, bool clip, const MmaRef &mma)
 {
     const int g = 2;
     const int m = min(H + 1 - l, l);
@@ -332,7 +332,7 @@ __device__ __forceinline__ HeadPlan head_plan(int H, int iters)
 // The result lands in bufs.WA, zero padded to whole tiles; returns an upper bound of its limb count.
 template <int T, bool MMA = false, bool CL = false>
 __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const ShinvBufs &bufs, Blk &blk,
-                                           bool clip, MmaCtx *mma = nullptr, int narrow_l = 0, bool seed = true,
+                                           bool clip, const MmaRef &mma = MmaRef{nullptr, 0, 0}, int narrow_l = 0, bool seed = true,
                                            const limb *wmid = nullptr)
 {
     limb *WA = bufs.WA, *WB = bufs.WB, *X = bufs.X, *P = bufs.P;
@@ -408,7 +408,7 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
         const int nlen = round_up(l + m + g + 2, TILE);
         if (T > 32 && l <= narrow_l && it + 2 < iters) {
             narrow_open = true;
-            if (threadIdx.x < 32) refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, nullptr);
+            if (threadIdx.x < 32) refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, clip, MmaRef{nullptr, 0, 0});
         } else {
             if (narrow_open) {                                 // leave the narrow phase: one block barrier,
                 narrow_open = false;                           // and a common collective parity again
@@ -464,7 +464,7 @@ __device__ __forceinline__ void shinv_head_warp(const limb *__restrict__ vg, int
     for (int it = SEED_ITERS; it < hp.it_end; ++it) {
         const int m = min(H + 1 - l, l);
         const int nlen = round_up(l + m + 2 + 2, TILE);
-        refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, true, nullptr);
+        refine_step<32>(V, k, H, it, l, wlen, Wc, Wn, X, P, ms, blk, true, MmaRef{nullptr, 0, 0});
         l = l + m - 1;
         wlen = nlen;
         limb *t = Wc; Wc = Wn; Wn = t;

@@ -260,23 +260,32 @@ __device__ __forceinline__ int mma_steps(int na, int nb, int dlo, int dhi)
 #ifndef MMA_PLAN_PCT
 #define MMA_PLAN_PCT 100
 #endif
+// What a caller needs to decide about the engine, by value: the context lives in memory (mma_mul_range is not inlined and
+// takes it by reference), and three dependent loads from it before every product were 3 % of a config-2 division.
+struct MmaRef {
+    MmaCtx *cx;      // nullptr: no engine for this instance
+    int cols;        // allocated TMEM columns
+    int cap;         // rows available for the row operand
+};
+
 template <int T>
-__device__ __forceinline__ bool mma_plan(const MmaCtx *cx, int na, int nb, int dlo, int dhi, bool &swap)
+__device__ __forceinline__ bool mma_plan(const MmaRef &m, int na, int nb, int dlo, int dhi, bool &swap)
 {
-    if (cx == nullptr || cx->fail || na <= 0 || nb <= 0 || dlo < 0) return false;
+    if (m.cx == nullptr || na <= 0 || nb <= 0 || dlo < 0) return false;
     dhi = min(dhi, (na + nb + 31) / 32);
     const int N = dhi - dlo, Nn = (N + 15) & ~15;
     if (N <= 0) return false;
     const int sa = mma_steps(na, nb, dlo, dhi), sb = mma_steps(nb, na, dlo, dhi);
     swap = sb < sa;
     const int steps = swap ? sb : sa;
-    if (steps <= 0 || Nn > cx->tmem_cols || Nn + steps - 1 > cx->brows_cap) return false;
+    if (steps <= 0 || Nn > m.cols || Nn + steps - 1 > m.cap) return false;
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
     const long long step_cycles = 4ll * max(max(32 + Nn / 4, Nn / 2), 40);
     const long long call_cycles = 2500ll + 20ll * Nn * (512 / T) + 6ll * (Nn + steps);
     const long long mma_cycles = steps * step_cycles + call_cycles;
     const long long imad_cycles = est * 512ll / (26ll * T);
-    return 100ll * imad_cycles >= (long long)MMA_PLAN_PCT * mma_cycles;
+    if (100ll * imad_cycles < (long long)MMA_PLAN_PCT * mma_cycles) return false;
+    return m.cx->fail == 0;                                      // a context whose pipeline gave up once is retired
 }
 
 // P[i] = limb 32*dlo + i of ((A * B) - E) mod B^(32 dhi), 0 <= E < B^(32 dlo + 1); i < 32 (dhi - dlo).

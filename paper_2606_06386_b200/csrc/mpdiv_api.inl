@@ -272,9 +272,9 @@ shinv_kernel(const limb *__restrict__ v, int v_limbs, int h, limb *__restrict__ 
             count(CNT_ONE_LIMB);
             if (threadIdx.x == 0) { V[1] = V[4]; V[4] = 0u; }   // v*B at the (aligned) base V
             __syncthreads();
-            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0, nullptr, narrow_l & 255, !(narrow_l & 256));
+            nw = shinv_block<T>(V, 1, h + 1, bufs, blk, clip != 0, MmaRef{nullptr, 0, 0}, narrow_l & 255, !(narrow_l & 256));
         } else {
-            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0, nullptr, narrow_l & 255, !(narrow_l & 256));
+            nw = shinv_block<T>(V + 4, pv - 1, h, bufs, blk, clip != 0, MmaRef{nullptr, 0, 0}, narrow_l & 255, !(narrow_l & 256));
         }
         store_number<T>(wout, bufs.WA, w_limbs, round_up(nw, TILE));
         __syncthreads();
@@ -432,8 +432,8 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         // short enough, the full one otherwise
         const bool compact = BIG || (mma != nullptr && max(h - k, 2) <= Lc.hcap);
         const DivLayout &Li = compact ? Lc : L;
-        MmaCtx *mma_i = (mma != nullptr && Li.mma_off >= 0) ? mma : nullptr;
-        if (mma_i) {                                       // the scratch of this instance's layout
+        const MmaRef mma_i{(mma != nullptr && Li.mma_off >= 0) ? mma : nullptr, Lc.mma_cols, Li.mma_rows};
+        if (mma_i.cx) {                                    // the scratch of this instance's layout
             mcx.brows = reinterpret_cast<uint8_t *>(smem + Li.mma_off);
             mcx.ring = mcx.brows + Li.mma_rows * 128;
             mcx.brows_cap = Li.mma_rows;
