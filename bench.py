@@ -546,6 +546,19 @@ def run_ours(args):
                 "div_per_s_128_thread_block_per_division": bs_ / (t_blk * 1e-3)}
             del dsu, dsv, qs, rs
         out["small_numbers_one_warp_per_division"] = small
+        # the same shapes at 8 times the batch: more waves per SM, so the head kernel amortises and the resident blocks of
+        # an SM drift out of lock step
+        big = {}
+        for cfg_, mult in ((2, 8), (3, 8), (4, 8)):
+            bb, mm, nn_ = inputs.CONFIG_SHAPES[cfg_]
+            ub, vb = inputs.uniform_operands(bb * mult, mm, nn_, config=30 + cfg_)
+            dbu, dbv = to_dev(ub), to_dev(vb)
+            qb, rb = torch.empty_like(dbu), torch.empty_like(dbv)
+            tb = float(np.median(time_steps(lambda: binding.mpdiv_batch(dbu, dbv, qb, rb), 5, 3, flush)))
+            big["config%d_shape_x%d" % (cfg_, mult)] = {"batch": bb * mult, "u_limbs": mm, "v_limbs": nn_, "div_ms": tb,
+                                                      "div_per_s": bb * mult / (tb * 1e-3)}
+            del dbu, dbv, qb, rb
+        out["larger_batches"] = big
         out["tensor_issue_probe"] = measure_mma_issue(binding)
         out["cpu_baseline"] = cpu_baseline(cfg)
         out["paper_context"] = "A100, 64-bit digits (PAPER.md:481-484): div/mul 6.77x/6.66x/6.94x/9.73x at 2^18..2^15 bits; model 5-7"
