@@ -84,17 +84,34 @@ __device__ __forceinline__ bool grp_or(bool pred)
     if (T == 32) return __any_sync(0xffffffffu, pred) != 0;
     return __syncthreads_or(pred) != 0;
 }
+// The per-warp words of a collective, through explicit shared-memory instructions (a volatile generic pointer compiles to
+// LD.E.STRONG.SYS / ST.E.STRONG.SYS).
+__device__ __forceinline__ uint32_t code_base(const Blk &blk)
+{
+    return (uint32_t)__cvta_generic_to_shared(blk.sc->code[blk.parity & 1]);
+}
+__device__ __forceinline__ void code_put(uint32_t base, uint32_t idx, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(base + 4u * idx), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t code_get(uint32_t base, uint32_t idx)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(base + 4u * idx) : "memory");
+    return v;
+}
+
 template <int T>
 __device__ __forceinline__ int block_max(int v, Blk &blk)
 {
     constexpr int NW = T / 32;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     v = __reduce_max_sync(0xffffffffu, v);
-    volatile uint32_t *code = blk.sc->code[blk.parity & 1];
+    const uint32_t code = code_base(blk);
     blk.parity++;
-    if (lane == 0) code[warp] = (uint32_t)v;
+    if (lane == 0) code_put(code, warp, (uint32_t)v);
     grp_sync<T>();
-    int r = (lane < NW) ? (int)code[lane] : INT32_MIN;
+    int r = (lane < NW) ? (int)code_get(code, lane) : INT32_MIN;
     return __reduce_max_sync(0xffffffffu, r);
 }
 
@@ -112,11 +129,11 @@ __device__ __forceinline__ uint32_t carry_scan(uint32_t g, uint32_t p, uint32_t 
     const uint32_t a = G | P, b = G;
     const uint32_t wg = (uint32_t)(((uint64_t)a + b) >> 32);   // warp generates
     const uint32_t wp = (P == 0xffffffffu) ? 2u : 0u;          // warp propagates
-    volatile uint32_t *code = blk.sc->code[blk.parity & 1];
+    const uint32_t code = code_base(blk);
     blk.parity++;
-    if (lane == 0) code[warp] = wg | wp;
+    if (lane == 0) code_put(code, warp, wg | wp);
     grp_sync<T>();
-    const uint32_t c = (lane < NW) ? code[lane] : 0u;
+    const uint32_t c = (lane < NW) ? code_get(code, lane) : 0u;
     const uint64_t GW = __ballot_sync(0xffffffffu, (c & 1u) != 0);
     const uint64_t PW = __ballot_sync(0xffffffffu, (c & 2u) != 0);
     const uint64_t aw = GW | PW, bw = GW;
@@ -223,37 +240,49 @@ __device__ __forceinline__ bool all_eq8(const limb (&r)[8], limb x)
 // materialised.  Map-scan-map of PAPER.md:423-432.  Returns the final carry (borrow).
 // dst may alias an operand only when that operand is read at the same index it is written.
 // Ends with a __syncthreads: dst is visible to the whole block on return.
+// one chunk of lin_addsub: r = fa +/- fb over limbs i0 .. i0 + 7; g = carry (borrow) out, p = an incoming one passes through
+template <bool SUB, class FA, class FB>
+__device__ __forceinline__ void lin_chunk(limb (&r)[8], uint32_t &g, uint32_t &p, int i0, const FA &fa, const FB &fb)
+{
+    limb a[8], b[8];
+#pragma unroll
+    for (int j = 0; j < 8; j++) {
+        a[j] = fa(i0 + j);
+        b[j] = fb(i0 + j);
+    }
+    if (SUB) {
+        g = sub8(r, a, b);
+        p = all_eq8(r, 0u);
+    } else {
+        g = add8(r, a, b);
+        p = all_eq8(r, 0xffffffffu);
+    }
+}
+template <bool SUB>
+__device__ __forceinline__ void lin_finish(limb *dst, limb (&r)[8], uint32_t c)
+{
+    if (SUB) dec8(r, c); else inc8(r, c);
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+    d4[0] = make_uint4(r[0], r[1], r[2], r[3]);
+    d4[1] = make_uint4(r[4], r[5], r[6], r[7]);
+}
+
+// (A form in which warp 0 also takes up to 32 tail chunks in the same scan -- the operands of a division are a few guard
+// limbs longer than 8 T, so full-size operations need a second pass for a handful of limbs -- was measured and lost
+// 2 % even at a single call site, 19 % everywhere: the inlined code doubles.)
 template <int T, bool SUB, class FA, class FB>
 __device__ __forceinline__ uint32_t lin_addsub(limb *dst, int len, FA fa, FB fb, uint32_t cin,
                                                Blk &blk)
 {
     for (int base = 0; base < len; base += CHUNK * T) {
         const int i0 = base + CHUNK * (int)threadIdx.x;
-        limb a[8], b[8], r[8];
+        limb r[8];
         const bool active = i0 < len;
         uint32_t g = 0, p = active ? 0u : 1u;   // idle threads pass the carry on to the block's cout
-        if (active) {
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                a[j] = fa(i0 + j);
-                b[j] = fb(i0 + j);
-            }
-            if (SUB) {
-                g = sub8(r, a, b);
-                p = all_eq8(r, 0u);
-            } else {
-                g = add8(r, a, b);
-                p = all_eq8(r, 0xffffffffu);
-            }
-        }
+        if (active) lin_chunk<SUB>(r, g, p, i0, fa, fb);
         uint32_t cout;
         const uint32_t c = carry_scan<T>(g, p, cin, blk, cout);
-        if (active) {
-            if (SUB) dec8(r, c); else inc8(r, c);
-            uint4 *d4 = reinterpret_cast<uint4 *>(dst + i0);
-            d4[0] = make_uint4(r[0], r[1], r[2], r[3]);
-            d4[1] = make_uint4(r[4], r[5], r[6], r[7]);
-        }
+        if (active) lin_finish<SUB>(dst + i0, r, c);
         cin = cout;
     }
     grp_sync<T>();

@@ -38,11 +38,18 @@ __device__ __forceinline__ void count_tiles(Blk &blk)
 }
 
 // significant limbs of a shared-memory number known to have at most `bound` limbs.
-// Every thread walks the same (stable) words, so the result is block-uniform.
+// Every warp scans the same (stable) words from the top, 32 per step (lane j looks at limb bound - 1 - j), so the
+// result is block-uniform without a barrier; the calling warps must be converged.
 __device__ __forceinline__ int top_prec(const limb *a, int bound)
 {
-    while (bound > 0 && a[bound - 1] == 0u) --bound;
-    return bound;
+    const int lane = (int)(threadIdx.x & 31);
+    while (bound > 0) {
+        const int i = bound - 1 - lane;
+        const uint32_t nz = __ballot_sync(0xffffffffu, i >= 0 && a[i] != 0u);
+        if (nz) return bound - (__ffs(nz) - 1);
+        bound -= 32;
+    }
+    return 0;
 }
 
 struct UnitView {   // B^pos
