@@ -447,28 +447,41 @@ __device__ __noinline__ int mma_mul_range(MmaCtx &cx_mem, const limb *A, int na,
     __syncthreads();
     tc_fence_after();
     {
+        // The four byte-column sums of a limb sit in lanes 8 apart of one lane quarter, i.e. of one warp.  They are
+        // brought together through the warp's own 2 KB of the engine's scratch (dead once the MMAs are done) instead of
+        // by shuffles: lane (b, j) stores the 16 columns it holds at [column][j][b], conflict free, and reads back the
+        // four words of (column, limb) pairs as one 16-byte load -- 64 shuffles per 16 columns made the epilogue
+        // shuffle-bound (a third of an SM's shuffle rate with four resident blocks).
         const int lane = tid & 31, quarter = warp & 3;
-        const int bsh = 8 * (lane >> 3);                           // byte of the limb this lane holds
-        const int limb_in_block = quarter + 4 * (7 - (lane & 7));  // (i div 4) for i = g + 16 (7 - r), g = 4 quarter + lane / 8
-        for (int d0 = 16 * (warp >> 2); d0 < Nn; d0 += 16 * (T / 128)) {
-            uint32_t v[16];
-            tmem_ld16(cx.tmem_base + ((uint32_t)(32 * quarter) << 16) + d0, v);
-            if (ni == 2) {                                            // the second issuer's accumulator set
-                uint32_t v2[16];
-                tmem_ld16(cx.tmem_base + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(Nn + d0), v2);
+        const int groups = min(T / 128, mma_scratch_bytes(cx.brows_cap, T) / 8192);     // 4 warps x 2 KB each
+        uint32_t *S = reinterpret_cast<uint32_t *>(cx.brows) + 512 * warp;
+        if ((warp >> 2) < groups) {
+            for (int d0 = 16 * (warp >> 2); d0 < Nn; d0 += 16 * groups) {
+                uint32_t v[16];
+                tmem_ld16(cx.tmem_base + ((uint32_t)(32 * quarter) << 16) + d0, v);
+                if (ni == 2) {                                            // the second issuer's accumulator set
+                    uint32_t v2[16];
+                    tmem_ld16(cx.tmem_base + ((uint32_t)(32 * quarter) << 16) + (uint32_t)(Nn + d0), v2);
 #pragma unroll
-                for (int k = 0; k < 16; ++k) v[k] += v2[k];
-            }
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                unsigned long long sv = (unsigned long long)v[k] << bsh;
-                sv += __shfl_xor_sync(0xffffffffu, sv, 8);
-                sv += __shfl_xor_sync(0xffffffffu, sv, 16);
-                if (lane < 8 && d0 + k < N) {
-                    const int L = 32 * (d0 + k) + limb_in_block;
-                    P[L] = (uint32_t)sv;
-                    HI[L + 1] = (uint32_t)(sv >> 32);
+                    for (int k = 0; k < 16; ++k) v[k] += v2[k];
                 }
+                uint32_t *Sw = S + (lane & 7) * 4 + (lane >> 3);          // [k][j = lane % 8][b = lane / 8]
+#pragma unroll
+                for (int k = 0; k < 16; ++k) Sw[32 * k] = v[k];
+                __syncwarp();
+#pragma unroll
+                for (int s4 = 0; s4 < 4; ++s4) {
+                    const int k = (lane >> 3) + 4 * s4, jj = lane & 7;    // item lane + 32 s4: words [k][jj][0..3]
+                    const uint4 w = *reinterpret_cast<const uint4 *>(S + 4 * lane + 128 * s4);
+                    const unsigned long long sv = (unsigned long long)w.x + ((unsigned long long)w.y << 8) +
+                                                  ((unsigned long long)w.z << 16) + ((unsigned long long)w.w << 24);
+                    if (d0 + k < N) {
+                        const int L = 32 * (d0 + k) + quarter + 4 * (7 - jj);   // (i div 4) for i = g + 16 (7 - r)
+                        P[L] = (uint32_t)sv;
+                        HI[L + 1] = (uint32_t)(sv >> 32);
+                    }
+                }
+                __syncwarp();
             }
         }
         if (tid == 0) HI[0] = 0u;
