@@ -340,6 +340,20 @@ __device__ __forceinline__ bool any_nonzero(const limb *a, int lo, int hi)
     return grp_or<T>(acc != 0);
 }
 
+// a >= b for a of `len` limbs and b of nb <= len limbs (zero above): the less-than of PAPER.md:331-335 as ONE reduction --
+// the highest limb in which the numbers differ decides -- instead of a subtraction with a borrow scan whose
+// result would be thrown away.  Block-uniform; one block barrier.
+template <int T>
+__device__ __forceinline__ bool big_ge(const limb *a, int len, const limb *b, int nb, Blk &blk)
+{
+    int top = -1;
+    for (int i = threadIdx.x; i < len; i += T)
+        if (a[i] != (i < nb ? b[i] : 0u)) top = i;    // i increases: the last hit is this thread's highest
+    top = block_max<T>(top, blk);
+    if (top < 0) return true;
+    return a[top] > (top < nb ? b[top] : 0u);
+}
+
 // number of significant limbs of a[0, n)  ("prec")
 template <int T>
 __device__ __forceinline__ int prec_of(const limb *a, int n, Blk &blk)

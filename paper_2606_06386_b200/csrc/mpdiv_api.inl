@@ -569,11 +569,17 @@ mpdiv_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v
         if (minus > 1) count(CNT_DELTA_NEG_MULTI);
         int plus = 0;
         for (int step = 0; step < CORR_MAX; ++step) {      // r >= v: delta = +1 (once by Theorem 2 as printed)
-            const uint32_t borrow =
-                lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
-            if (borrow) break;
+            if (!big_ge<T>(R, rlen, Vb, k + 1, blk)) break;     // the comparison alone: no subtraction to throw away
+            lin_addsub<T, true>(R2, rlen, LimbView{R, rlen, 0}, LimbView{Vb, k + 1, 0}, 0u, blk);
             limb *t = R; R = R2; R2 = t;
-            lin_addsub<T, false>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+            const limb qlow = Q[0];
+            __syncthreads();                               // every thread has read the limb before it changes
+            if (qlow != 0xffffffffu) {                     // q + 1 without a carry: one limb
+                if (threadIdx.x == 0) Q[0] = qlow + 1u;
+                __syncthreads();
+            } else {
+                lin_addsub<T, false>(Q, qlen, LimbView{Q, qlen, 0}, ZeroView{}, 1u, blk);
+            }
             ++plus;
         }
         if (plus == 1) count(CNT_DELTA_POS);
