@@ -347,8 +347,9 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     const int g = 2;
 
     // ---- special cases (Alg. 1 lines 5-10) -------------------------------------
-    const bool low_nz = any_nonzero<T>(V, 0, k);
     const limb vtop = V[k];
+    // the limbs below the top one only matter when the top limb is 1 (v = B^k?) or 2^31 (2v > B^h?)
+    const bool low_nz = (vtop == 1u || vtop == 0x80000000u) ? any_nonzero<T>(V, 0, k) : true;
     const bool pow_b = (vtop == 1u) && !low_nz;               // v = B^k
     int special = -1;                                          // value of a one-limb result
     if (k > h || (k == h && !pow_b)) special = 0;              // v > B^h
