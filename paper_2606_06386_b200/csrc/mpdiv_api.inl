@@ -707,7 +707,7 @@ static cudaMemPool_t head_pool()
 
 // A thread-block cluster per division (mpdiv_kernel<128, true, false, false, true>): for batches so small that
 // clusters of `cs` CTAs still run all at once.  Returns the largest admissible size in {8, 4, 2} (at most cap), or 1.
-static int cluster_size_for(int batch, int cap, size_t bytes)
+static int cluster_size_query(int batch, int cap, size_t bytes)
 {
     for (int cs = 8; cs >= 2; cs /= 2) {
         if (cs > cap || batch * cs > g_sm_count) continue;
@@ -730,6 +730,23 @@ static int cluster_size_for(int batch, int cap, size_t bytes)
         if (nact >= batch) return cs;
     }
     return 1;
+}
+
+static int cluster_size_for(int batch, int cap, size_t bytes)
+{
+    // the answer for the last question asked on each device is kept: the occupancy query costs tens of microseconds of
+    // host time, and the batches that come here are the latency-bound ones
+    struct Memo { int batch, cap, cs; size_t bytes; };
+    static Memo memo[MAX_DEVICES] = {};
+    {
+        std::lock_guard<std::mutex> lk(g_host_mutex);
+        const Memo &m = memo[g_dev];
+        if (m.cs && m.batch == batch && m.cap == cap && m.bytes == bytes) return m.cs;
+    }
+    const int cs = cluster_size_query(batch, cap, bytes);
+    std::lock_guard<std::mutex> lk(g_host_mutex);
+    memo[g_dev] = Memo{batch, cap, cs, bytes};
+    return cs;
 }
 
 static int launch_div_cluster(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q, limb *r, int batch,
