@@ -430,7 +430,9 @@ template <int T, bool CL>
 __device__ __forceinline__ void mul_phases(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd, int Kc, limb *Pd,
                                            limb *HId, uint32_t *OVd, uint32_t *C3d, const MulScratch &ms, Blk &blk, bool snake)
 {
-    if constexpr (CL) {
+    // cluster form: a product of so few diagonals that one CTA covers them in a single pass is computed by every CTA
+    // for itself (the state is replicated): the barrier and the remote stores would cost more than the share saves
+    if (CL && (Kd - Klo) * 4 > T) {
         const int cap = ms.stage_cap;
         limb *S = ms.ST + ((blk.cl >> 16) & 1u) * (uint32_t)stage_set_words(cap);
         limb *Ps = S - TILE * Klo, *HIs = S + cap - TILE * Klo;
