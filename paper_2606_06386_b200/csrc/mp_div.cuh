@@ -384,8 +384,12 @@ __device__ __forceinline__ int shinv_block(const limb *V, int k, int h, const Sh
     const HeadPlan hp = (clip && wmid) ? head_plan(H, iters) : HeadPlan{0, 0, 0};
     if (hp.it_end) {
         // the head kernel left the iterate after it_end iterations in the workspace row
+        // The division kernel is launched with programmatic stream serialisation behind the head kernel: its blocks
+        // start while the head still runs (their set-up, loads and precisions need nothing from it) and wait HERE for
+        // the head grid to have completed and flushed its rows.
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         if (hp.it_end & 1) { limb *t = Wc; Wc = Wn; Wn = t; }
-        for (int i = threadIdx.x; i < hp.wlen_end; i += T) Wc[i] = __ldg(wmid + i);
+        for (int i = threadIdx.x; i < hp.wlen_end; i += T) Wc[i] = __ldcg(wmid + i);
         l = hp.l_end;
         wlen = hp.wlen_end;
         it0 = hp.it_end;

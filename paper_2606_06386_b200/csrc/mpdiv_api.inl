@@ -232,6 +232,7 @@ shinv_head_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restric
                   limb *__restrict__ wmid, int batch)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
+    asm volatile("griddepcontrol.launch_dependents;");     // the division kernel may start its blocks (see shinv_block)
     const int inst = blockIdx.x;
     if (inst >= batch) return;
     const int h = warp_prec(u + (size_t)inst * u_limbs, u_limbs);
@@ -814,8 +815,27 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
             shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
         }
     }
-    mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid, 0);
-    const bool ok = cudaGetLastError() == cudaSuccess;
+    bool ok;
+    if (wmid) {
+        // behind a head kernel: programmatic stream serialisation (the blocks wait for the head grid inside shinv_block)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)batch);
+        cfg.blockDim = dim3(T);
+        cfg.dynamicSmemBytes = bytes;
+        cfg.stream = st;
+        cudaLaunchAttribute at;
+        at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at.val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = &at;
+        cfg.numAttrs = 1;
+        const limb *wm = wmid;
+        ok = cudaLaunchKernelEx(&cfg, mpdiv_kernel<T, LAT, MMA>, u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip,
+                                narrow_for(sched, tn), wm, 0) == cudaSuccess;
+        if (!ok) cudaGetLastError();
+    } else {
+        mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid, 0);
+        ok = cudaGetLastError() == cudaSuccess;
+    }
     if (wmid && !tn.wmid_fixed) cudaFreeAsync(wmid, st);
     return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
