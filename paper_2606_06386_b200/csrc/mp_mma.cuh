@@ -282,7 +282,9 @@ __device__ __forceinline__ bool mma_plan(const MmaRef &m, int na, int nb, int dl
     const long long est = (long long)(32 * N) * (long long)min(na, nb);      // limb products, upper bound
     const long long step_cycles = 4ll * max(max(32 + Nn / 4, Nn / 2), 40);
     const long long call_cycles = 2500ll + 20ll * Nn * (512 / T) + 6ll * (Nn + steps);
-    const long long mma_cycles = steps * step_cycles + call_cycles;
+    // the blocks of an SM run in lock step and enter their MMA loops together: the unit is shared by 512 / T of them,
+    // just as the IMAD pipe is (config 2: a 33-step band product took 21 000 cycles on the shared unit, ~11 000 on IMAD)
+    const long long mma_cycles = steps * step_cycles * (512 / T) + call_cycles;
     const long long imad_cycles = est * 512ll / (26ll * T);
     if (100ll * imad_cycles < (long long)MMA_PLAN_PCT * mma_cycles) return false;
     return m.cx->fail == 0;                                      // a context whose pipeline gave up once is retired
