@@ -71,8 +71,12 @@ enum {
  * (mpdiv_batch_launches() == 2) runs the short-operand head of Refine in a kernel of its own first, one
  * warp per division, and passes its iterate (batch x 272 limbs) through a stream-ordered allocation from a
  * library-owned memory pool of the current device (created on first use, never destroyed; freed rows stay
- * in the pool).  Everything is enqueued on `stream`; nothing synchronises.
+ * in the pool).  The division kernel is launched behind that head kernel with programmatic stream serialisation:
+ * its blocks start while the head still runs and wait for it (griddepcontrol.wait) where they take its rows over.
+ * Everything is enqueued on `stream`; nothing synchronises.
  * Rows travel between HBM and shared memory as 1-D bulk asynchronous copies (cp.async.bulk + mbarrier).
+ * A batch of at most half as many divisions as the GPU has SMs, of 1024 limbs or more, runs every division on a
+ * thread-block cluster of 2-4 CTAs; small numbers in large batches run one division per warp.
  * MPDIV_MAX_OPERAND_LIMBS < u_limbs <= MPDIV_MAX_LIMBS (2^19 bits; v_limbs <= MPDIV_MAX_OPERAND_LIMBS): the dividend
  * stays in HBM.  The quotient is produced t = 2048 limbs at a time (1024 or 512 if shared memory is short) from a
  * window x = r' B^t + (next t limbs of u), r' the running remainder: x < v B^t, so one shifted inverse
