@@ -252,7 +252,11 @@ __device__ __forceinline__ void cluster_st1(uint32_t addr, uint32_t a)
 // A pass that has fewer diagonals left than groups widens its groups (up to a whole warp).
 // CL: the cluster form (above): crank / csize = this CTA's rank in its cluster and the cluster's size; P, HI, OV are the
 // staging set of this product.
-template <int T, bool CL>
+// COMPACT: one copy of the 64-product tile in a plain loop instead of two in a ping-pong loop plus a tail copy.  A
+// latency-bound division runs ONE warp per scheduler through code that is cold at every call (a tile is ~165
+// instructions = 21 lines of instruction cache): at config 1 a tile then costs ~750 cycles of instruction fetch against
+// ~300 once its code is resident, so fewer copies of it beat the hidden operand latency of the ping-pong form.
+template <int T, bool CL, bool COMPACT = false>
 __device__ __forceinline__ uint32_t mul_diagonals_body(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
                                                        limb *P, limb *HI, uint32_t *OV, bool snake, int crank, int csize)
 {   // everything by value: a reference argument of a noinline function lives in local memory
@@ -289,6 +293,15 @@ __device__ __forceinline__ uint32_t mul_diagonals_body(const limb *A, int Na, co
             const int step = 4 * TILE * C;                  // bytes between a lane's consecutive tiles
             uint32_t pa = (uint32_t)__cvta_generic_to_shared(A) + 4 * TILE * I;
             uint32_t pb = (uint32_t)__cvta_generic_to_shared(Bp) + 4 * TILE * (K - I);
+            if (COMPACT) {
+#pragma unroll 1
+                for (; I <= Ihi; I += C) {
+                    load_tile(a0, pa);
+                    load_tile(b0, pb);
+                    pa += step; pb -= step;
+                    tile_mac(s, a0, b0);
+                }
+            } else {
             load_tile(a0, pa);
             load_tile(b0, pb);
             // two tiles per trip with ping-pong operand registers (no register copies)
@@ -305,6 +318,7 @@ __device__ __forceinline__ uint32_t mul_diagonals_body(const limb *A, int Na, co
                 tile_mac(s, a1, b1);
             }
             if (I <= Ihi) tile_mac(s, a0, b0);
+            }
         }
         uint32_t d[17];
         diag_finish(s, d);
@@ -353,7 +367,13 @@ template <int T>
 __device__ __noinline__ uint32_t mul_diagonals_cluster(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
                                                        limb *P, limb *HI, uint32_t *OV, bool snake, int crank, int csize)
 {
-    return mul_diagonals_body<T, true>(A, Na, Bp, Nb, Klo, Kd, P, HI, OV, snake, crank, csize);
+    return mul_diagonals_body<T, true, true>(A, Na, Bp, Nb, Klo, Kd, P, HI, OV, snake, crank, csize);
+}
+template <int T>
+__device__ __noinline__ uint32_t mul_diagonals_compact(const limb *A, int Na, const limb *Bp, int Nb, int Klo, int Kd,
+                                                       limb *P, limb *HI, uint32_t *OV, bool snake)
+{
+    return mul_diagonals_body<T, false, true>(A, Na, Bp, Nb, Klo, Kd, P, HI, OV, snake, 0, 1);
 }
 
 // Phase 2: resolve column blocks Klo..Kc-1 in place: P[K] = P[K] + HI[K-1] + OV[K-2] + carries,
@@ -442,7 +462,8 @@ __device__ __forceinline__ void mul_phases(const limb *A, int Na, const limb *Bp
         blk.parity = mul_resolve_cluster<T>(Pd, Ps, Klo, Kd, Kc, HIs, OVs, C3d, blk);
         blk.cl ^= 1u << 16;
     } else {
-        blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, snake);
+        if (CL) blk.tiles += mul_diagonals_compact<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, snake);
+        else blk.tiles += mul_diagonals<T>(A, Na, Bp, Nb, Klo, Kd, Pd, HId, OVd, snake);
         blk.parity = mul_resolve<T>(Pd, Klo, Kd, Kc, HId, OVd, C3d, blk);
     }
 }
