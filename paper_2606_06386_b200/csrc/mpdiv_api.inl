@@ -229,7 +229,7 @@ __device__ __forceinline__ int warp_prec(const limb *__restrict__ a, int n)
 
 __global__ void __launch_bounds__(32, 16)
 shinv_head_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restrict__ v, int v_limbs,
-                  limb *__restrict__ wmid, int batch)
+                  limb *__restrict__ wmid, int batch, int tchunk)
 {
     extern __shared__ __align__(1024) uint32_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");     // the division kernel may start its blocks (see shinv_block)
@@ -238,7 +238,9 @@ shinv_head_kernel(const limb *__restrict__ u, int u_limbs, const limb *__restric
     const int h = warp_prec(u + (size_t)inst * u_limbs, u_limbs);
     const int pv = warp_prec(v + (size_t)inst * v_limbs, v_limbs);
     if (pv < 2 || pv > h) return;                        // zero and one-limb divisors, u < v: the division kernel's own paths
-    shinv_head_warp(v + (size_t)inst * v_limbs, pv - 1, h, smem, wmid + (size_t)inst * WMID_STRIDE);
+    int hx = h;                                          // chunked form (tchunk > 0): the inverse all windows share
+    if (tchunk > 0 && (h - (pv - 1) + tchunk - 1) / tchunk > 1) hx = pv + tchunk;
+    shinv_head_warp(v + (size_t)inst * v_limbs, pv - 1, hx, smem, wmid + (size_t)inst * WMID_STRIDE);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -706,6 +708,45 @@ static cudaMemPool_t head_pool()
     return pools[dev];
 }
 
+// Runs the head of Refine for a batch in its own kernel and returns the rows it leaves its iterates in (the static
+// scratch of mpdiv_batch_noalloc, or a stream-ordered allocation the caller frees with cudaFreeAsync after the division
+// kernel); nullptr = no rows (no pool on this device): Refine stays in the block.
+static limb *run_head(const limb *u, int u_limbs, const limb *v, int v_limbs, int batch, cudaStream_t st, const Tune &tn,
+                      int tchunk)
+{
+    limb *wmid = tn.wmid_fixed;
+    if (!wmid && (!head_pool() ||
+                  cudaMallocFromPoolAsync(reinterpret_cast<void **>(&wmid), (size_t)batch * WMID_STRIDE * sizeof(limb), head_pool(),
+                                          st) != cudaSuccess)) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch, tchunk);
+    return wmid;
+}
+
+// Launches a division kernel behind the head kernel with programmatic stream serialisation: its blocks start while the
+// head still runs and wait for the head grid inside shinv_block (griddepcontrol.wait).
+template <class K, class... Args>
+static bool launch_behind_head(K kernel, int grid, int threads, size_t bytes, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute at;
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, kernel, args...) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return true;
+}
+
 // A thread-block cluster per division (mpdiv_kernel<128, true, false, false, true>): for batches so small that
 // clusters of `cs` CTAs still run all at once.  Returns the largest admissible size in {8, 4, 2} (at most cap), or 1.
 static int cluster_size_query(int batch, int cap, size_t bytes)
@@ -802,36 +843,12 @@ int launch_div_m(const limb *u, int u_limbs, const limb *v, int v_limbs, limb *q
     if (rc != MPDIV_OK) return rc;
     // throughput batches: the head of Refine runs in its own kernel, one warp per division, and hands the
     // iterate over in a stream-ordered workspace (mp_div.cuh "Head of Refine")
-    limb *wmid = nullptr;
-    if (use_head(u_limbs, clip, LAT, tn) && tn.wmid_fixed) {
-        wmid = tn.wmid_fixed;                                // mpdiv_batch_noalloc: the library's static scratch
-        shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
-    } else if (use_head(u_limbs, clip, LAT, tn)) {
-        if (!head_pool() ||
-            cudaMallocFromPoolAsync(reinterpret_cast<void **>(&wmid), (size_t)batch * WMID_STRIDE * sizeof(limb), head_pool(), st) != cudaSuccess) {
-            cudaGetLastError();
-            wmid = nullptr;                                  // no pool on this device: Refine stays in the block
-        } else {
-            shinv_head_kernel<<<batch, 32, HEAD_SMEM_WORDS * 4, st>>>(u, u_limbs, v, v_limbs, wmid, batch);
-        }
-    }
+    limb *wmid = use_head(u_limbs, clip, LAT, tn) ? run_head(u, u_limbs, v, v_limbs, batch, st, tn, 0) : nullptr;
     bool ok;
     if (wmid) {
-        // behind a head kernel: programmatic stream serialisation (the blocks wait for the head grid inside shinv_block)
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)batch);
-        cfg.blockDim = dim3(T);
-        cfg.dynamicSmemBytes = bytes;
-        cfg.stream = st;
-        cudaLaunchAttribute at;
-        at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at.val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = &at;
-        cfg.numAttrs = 1;
         const limb *wm = wmid;
-        ok = cudaLaunchKernelEx(&cfg, mpdiv_kernel<T, LAT, MMA>, u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip,
-                                narrow_for(sched, tn), wm, 0) == cudaSuccess;
-        if (!ok) cudaGetLastError();
+        ok = launch_behind_head(mpdiv_kernel<T, LAT, MMA>, batch, T, bytes, st, u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip,
+                                narrow_for(sched, tn), wm, 0);
     } else {
         mpdiv_kernel<T, LAT, MMA><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, Lc, clip, narrow_for(sched, tn), wmid, 0);
         ok = cudaGetLastError() == cudaSuccess;
@@ -857,9 +874,20 @@ int launch_div_big(const limb *u, int u_limbs, const limb *v, int v_limbs, limb 
     if (tn.no_mma) L.mma_off = -1;
     int rc = set_smem(mpdiv_kernel<T, false, true, true>, bytes);
     if (rc != MPDIV_OK) return rc;
-    mpdiv_kernel<T, false, true, true><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, L, 1, narrow_for(sched, tn),
-                                                                nullptr, t);
-    return cudaGetLastError() == cudaSuccess ? MPDIV_OK : MPDIV_ERR_CUDA;
+    // the head of Refine in its own kernel, as for the resident form: one warp per division instead of 512 threads
+    limb *wmid = (!tn.no_head && !tn.no_seed) ? run_head(u, u_limbs, v, v_limbs, batch, st, tn, t) : nullptr;
+    const limb *wm = wmid;
+    bool ok;
+    if (wmid) {
+        ok = launch_behind_head(mpdiv_kernel<T, false, true, true>, batch, T, bytes, st, u, u_limbs, v, v_limbs, q, r, batch, L, L, 1,
+                                narrow_for(sched, tn), wm, t);
+    } else {
+        mpdiv_kernel<T, false, true, true><<<batch, T, bytes, st>>>(u, u_limbs, v, v_limbs, q, r, batch, L, L, 1, narrow_for(sched, tn),
+                                                                    wm, t);
+        ok = cudaGetLastError() == cudaSuccess;
+    }
+    if (wmid && !tn.wmid_fixed) cudaFreeAsync(wmid, st);
+    return ok ? MPDIV_OK : MPDIV_ERR_CUDA;
 }
 
 template <int T, bool LAT>
@@ -1117,7 +1145,7 @@ int mpdiv_batch_launches(int u_limbs, int batch, int flags)
 {
     if (u_limbs <= 0 || batch <= 0 || !flags_ok(flags) || !device_props()) return 0;
     const Tune tn = tune_of(flags);
-    if (u_limbs > MPDIV_MAX_OPERAND_LIMBS) return 1;
+    if (u_limbs > MPDIV_MAX_OPERAND_LIMBS) return (!tn.no_head && !tn.no_seed) ? 2 : 1;
     const int T = threads_for(u_limbs, tn.threads, batch);
     const bool lat = T <= 256 && batch <= (T <= 128 ? 2 : 1) * g_sm_count;
     return use_head(u_limbs, (flags & MPDIV_VARIANT_MASK) == MPDIV_VARIANT_CLIPPED, lat, tn) ? 2 : 1;

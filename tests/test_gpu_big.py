@@ -69,6 +69,21 @@ def test_paper_shape_2p19():
     check(u, v, "paper shape 16384")
 
 
+def test_head_kernel_on_and_off_2p19():
+    """The head of Refine runs in its own kernel for the chunked form too (the inverse all windows share has t + 2 limbs:
+    the head must plan for H = t + 1, not for h - k); with MPDIV_FLAG_NO_HEAD everything stays in the block."""
+    assert binding.batch_launches(16384, 592) == 2
+    assert binding.batch_launches(16384, 592, binding.VARIANT_CLIPPED | binding.FLAG_NO_HEAD) == 1
+    u, v = inputs.directed(16384, 8192, count=64, seed=inputs.SEED + 5)
+    check(u, v, "directed 16384/8192, head in the block", flags=binding.VARIANT_CLIPPED | binding.FLAG_NO_HEAD)
+    check(u, v, "directed 16384/8192, no seed", flags=binding.VARIANT_CLIPPED | binding.FLAG_NO_SEED)
+    q = torch.empty((u.shape[0], 16384), dtype=torch.int32, device="cuda")
+    r = torch.empty((u.shape[0], 8192), dtype=torch.int32, device="cuda")
+    binding.mpdiv_batch_noalloc(dev(u), dev(v), q, r)                 # the static scratch serves the chunked form as well
+    qo, ro = oracle.divmod_batch(u, v, threads=NCPU)
+    assert (host(q) == qo).all() and (host(r) == ro).all() and binding.status(reset=True) == 0
+
+
 def test_no_tensor_engine_2p19():
     u, v = inputs.uniform_operands(8, 16384, 8192, config=20)
     check(u, v, "uniform 16384/8192, IMAD only", flags=binding.VARIANT_CLIPPED | binding.FLAG_NO_MMA)
